@@ -1,0 +1,183 @@
+/*
+ * aev.h -- C ABI of libaev_b200.so: the B200-native (sm_100a) hot path of an ANI-style
+ * ML-potential force evaluation inside an MD step.
+ *
+ * What the path is for: "a model that takes atomic positions as input and computes
+ * potential energy.  Forces can be automatically calculated through backpropagation, or
+ * ... returned explicitly" (section "OpenMM-Torch").  Which operations it
+ * consists of: "computing the atom-centered symmetry functions used in the ANI family of
+ * potentials, building neighbor lists" (section "Optimization Through
+ * NNPOps").  The paper prints no formulas; the formulas are BASELINE.json:north_star's
+ * steps (1)-(4) as restated in SURVEY.md section 8(c) and DESIGN.md section 3:
+ *
+ *   (1) pairs    d_ij = x_j - x_i - L*rint((x_j - x_i)/L)  (orthorhombic minimum image),
+ *                radial set r_ij < rcr, angular set r_ij < rca   (strict <)
+ *   (2) radial   G_R[i][s*nR+m]  = sum_{j in radial set, s_j=s}
+ *                                  0.25*exp(-eta_r*(r_ij-shf_r[m])^2)*fc(r_ij; rcr)
+ *   (3) angular  G_A[i][S*nR + p(s_j,s_k)*nA*nZ + a*nZ + z] = sum over UNORDERED {j,k} in
+ *                the angular set of
+ *                2^(1-zeta)*(1+cos(theta-shf_z[z]))^zeta*exp(-eta_a*((r_ij+r_ik)/2-shf_a[a])^2)
+ *                *fc(r_ij; rca)*fc(r_ik; rca),   theta = acos(cos_scale * cos(angle j-i-k)),
+ *                p(s1<=s2) = s1*(2S-s1-1)/2 + s2,   fc(r;R) = 0.5*cos(pi*r/R)+0.5
+ *   (4) backward forces[a] = - sum_i sum_slot grad_aev[i][slot] * dAEV[i][slot]/dx_a,
+ *                then per-species MLPs  z = hW+b, CELU_alpha hidden, linear last layer,
+ *                E = sum_i NN_{s_i}(AEV_i)                     (BASELINE.json:configs[4])
+ *
+ * Conventions for every call
+ *   - plain pointers and sizes only; "device" pointers are CUDA device pointers on the
+ *     context's device, "host" pointers are ordinary host memory;
+ *   - the caller owns every buffer passed in; the library never frees them and keeps no
+ *     pointer to them after the call returns (it copies what aev_backward needs into
+ *     workspace owned by the context);
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *     device-pointer calls are asynchronous on that stream unless marked "syncs";
+ *   - every call returns 0 (AEV_OK) or a negative AEV_ERR_* code; nothing throws, prints
+ *     or exits;
+ *   - a context is used from one host thread and one stream at a time;
+ *   - there is no CPU fallback and no other backend: a device that is not compute
+ *     capability 10.x gives AEV_ERR_UNSUPPORTED.
+ *
+ * Supported parameter space (else AEV_ERR_UNSUPPORTED): 1 <= num_species <= 8,
+ * n_shf_r == 16, n_shf_a == 4, n_shf_z == 8 (the ANI-1x/2x shapes, BASELINE.json:configs[0]),
+ * zeta a power of two in [1,64], 0 < rca <= rcr, 0 < cos_scale <= 1, orthorhombic boxes.
+ */
+#ifndef AEV_B200_H
+#define AEV_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    AEV_OK = 0,
+    AEV_ERR_INVALID_ARG = -1,   /* null pointer, bad shape, n > max_atoms, ...                 */
+    AEV_ERR_BOX_TOO_SMALL = -2, /* a periodic edge < 2*rcr (no unique minimum image) or < 3 cells */
+    AEV_ERR_CAPACITY = -3,      /* a per-atom neighbour capacity or a cell capacity overflowed
+                                   on the device; results of that call are incomplete          */
+    AEV_ERR_STATE = -4,         /* aev_backward without a preceding aev_forward, MLP not loaded */
+    AEV_ERR_UNSUPPORTED = -5,   /* parameter combination or device outside the supported space  */
+    AEV_ERR_CUDA = -6           /* a CUDA runtime call failed                                   */
+};
+
+typedef struct aev_ctx aev_ctx; /* opaque; owns all device workspace */
+
+typedef struct {
+    int32_t num_species;        /* S; species ids are 0..S-1, id < 0 marks a padding atom       */
+    float rcr, rca;             /* radial / angular cutoff, same length unit as positions       */
+    float eta_r;
+    int32_t n_shf_r;
+    const float *shf_r;         /* HOST pointer, n_shf_r values, copied at create               */
+    float eta_a, zeta;
+    int32_t n_shf_a;
+    const float *shf_a;         /* HOST, n_shf_a values                                         */
+    int32_t n_shf_z;
+    const float *shf_z;         /* HOST, n_shf_z values (radians)                               */
+    float cos_scale;            /* 1.0 = the literal north_star formula; 0.95 = damped variant  */
+    int32_t max_atoms;          /* capacity: atoms per system                                   */
+    int32_t max_batch;          /* capacity: systems per call                                   */
+    int32_t max_radial_nbrs;    /* per-atom capacity for r < rcr (0 = default 128)              */
+    int32_t max_angular_nbrs;   /* per-atom capacity for r < rca (0 = default 48; <= 64)        */
+    int32_t device;             /* CUDA ordinal                                                 */
+} aev_params;
+
+/* Creates a context (allocates workspace for max_batch*max_atoms atoms on `device`). Syncs. */
+int aev_create(const aev_params *p, aev_ctx **out);
+/* Frees the context and everything it owns. Syncs. NULL is accepted. */
+int aev_destroy(aev_ctx *c);
+/* L = S*n_shf_r + S*(S+1)/2*n_shf_a*n_shf_z (384 for S = 4). Negative on a NULL context. */
+int aev_length(const aev_ctx *c);
+
+/*
+ * Step (1) only: cutoff neighbour search.
+ *   pos      device f32 [batch][n_atoms][3]
+ *   species  device i32 [batch][n_atoms]; id < 0 = padding atom (belongs to no pair)
+ *   box      HOST f32[3] orthorhombic edge lengths (shared by the batch), or NULL =
+ *            non-periodic all-pairs within each system.  Positions may lie outside [0,L).
+ * Builds, inside the context, per-atom neighbour lists (angular-set neighbours first) that
+ * aev_export_pairs can read back.  Asynchronous.
+ */
+int aev_neighbors(aev_ctx *c, const float *pos, const int32_t *species, const float *box,
+                  int32_t n_atoms, int32_t batch, void *stream);
+
+/*
+ * Steps (1)-(3): neighbour search (always rebuilt, reading G18) + radial and
+ * angular AEV (rows A1-A4).
+ *   aev_out  device f32 [batch][n_atoms][L], OVERWRITTEN, rows in the caller's atom order;
+ *            rows of padding atoms are written as zeros.
+ * Keeps what aev_backward needs inside the context.  Asynchronous.
+ */
+int aev_forward(aev_ctx *c, const float *pos, const int32_t *species, const float *box,
+                int32_t n_atoms, int32_t batch, float *aev_out, void *stream);
+
+/*
+ * Step (4), first half (rows A5-A7), for the most recent aev_forward on this context:
+ *   grad_aev    device f32 [batch][n_atoms][L]  upstream dE/dAEV
+ *   forces_out  device f32 [batch][n_atoms][3], OVERWRITTEN,
+ *               forces_out[a] = - sum_i sum_slot grad_aev[i][slot]*dAEV[i][slot]/dx_a
+ * No global atomics: per-pair gradients are gathered, so results are run-to-run identical.
+ * AEV_ERR_STATE if no forward precedes it.  Asynchronous.
+ */
+int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *stream);
+
+/*
+ * Loads the network of one species (rows A8-A9; BASELINE.json:configs[4]).
+ *   dims     HOST i32 [n_layers+1]; dims[0] must equal L, dims[n_layers] must be 1,
+ *            2 <= n_layers <= 4, hidden widths multiples of 16 and <= 256
+ *   weights  HOST array of n_layers HOST pointers, layer l is f32 [dims[l]][dims[l+1]]
+ *            row-major ("[in][out]"); weights are used as their bf16 hi+lo split
+ *   biases   HOST array of n_layers HOST pointers, f32 [dims[l+1]]
+ * Hidden activations are CELU(alpha); the last layer is linear.  Syncs.
+ */
+int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const int32_t *dims,
+                 const float *const *weights, const float *const *biases, float celu_alpha);
+
+/*
+ * The whole path: neighbours + AEV + per-species MLP forward/backward + AEV backward.
+ *   energy_out  device f64 [batch]             E_b = sum_i NN_{s_i}(AEV_i)
+ *   forces_out  device f32 [batch][n_atoms][3]  -dE/dx
+ * Every species present must have a network loaded (else the device flag reports
+ * AEV_ERR_STATE through aev_status).  Asynchronous.
+ */
+int ani_energy_forces(aev_ctx *c, const float *pos, const int32_t *species, const float *box,
+                      int32_t n_atoms, int32_t batch, double *energy_out, float *forces_out,
+                      void *stream);
+
+/*
+ * Host-buffer convenience entry points (the "end to end" calls bench.py times): every
+ * pointer is a HOST pointer; the library stages through pinned buffers and device
+ * workspace it owns, runs the same kernels, and copies the results back.  They sync.
+ * Any of aev_out / grad_aev+forces_out may be NULL to skip that half.
+ */
+int aev_forward_backward_host(aev_ctx *c, const float *pos, const int32_t *species,
+                              const float *box, int32_t n_atoms, int32_t batch,
+                              const float *grad_aev, float *aev_out, float *forces_out);
+int ani_energy_forces_host(aev_ctx *c, const float *pos, const int32_t *species,
+                           const float *box, int32_t n_atoms, int32_t batch,
+                           double *energy_out, float *forces_out);
+
+/*
+ * Test / diagnostic exports.
+ * aev_export_pairs: the undirected pair set of the last neighbour build as (i<j) in the
+ * caller's FLAT atom index (b*n_atoms + a), in no particular order.
+ *   which      0 = radial set (r < rcr), 1 = angular set (r < rca)
+ *   pairs_out  device i32 [cap][2];  count_out HOST i64 = pairs found (may exceed cap; only
+ *              the first cap are written).  Syncs.
+ */
+int aev_export_pairs(aev_ctx *c, int32_t which, int32_t *pairs_out, int64_t cap,
+                     int64_t *count_out);
+/* Syncs the context's last stream and returns AEV_OK or the deferred device-side error
+ * (AEV_ERR_CAPACITY, AEV_ERR_STATE) raised by any call since the last aev_status. */
+int aev_status(aev_ctx *c);
+/* Number of kernels the library has launched on this context so far (bench bookkeeping). */
+int64_t aev_launch_count(const aev_ctx *c);
+/* Independent-FMA microbenchmark: measured FP32 FMA throughput of `device` in TFLOP/s
+ * (the ALU roofline denominator).  Syncs. */
+int aev_probe_fp32_tflops(int32_t device, double *tflops_out);
+const char *aev_error_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AEV_B200_H */

@@ -1,0 +1,287 @@
+"""Thin ctypes binding of libaev_b200.so (include/aev.h) -- argument marshalling only.
+
+Every step of the path (neighbour search, AEV forward/backward, per-species MLPs) runs in
+the CUDA kernels of `csrc/`; PyTorch is used here for device memory and streams only.
+There is no CPU fallback: loading fails loudly if the library is missing, and every call
+raises `AevError` on a non-zero return code.  This package never imports `oracle`.
+
+The functions carry the names of the C ABI (PAPER.md:75 contract; BASELINE.json:north_star
+entry points): aev_create, aev_neighbors, aev_forward, aev_backward, ani_mlp_load,
+ani_energy_forces, aev_export_pairs, aev_status.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaev_b200.so")
+
+AEV_OK = 0
+ERRORS = {
+    -1: "AEV_ERR_INVALID_ARG", -2: "AEV_ERR_BOX_TOO_SMALL", -3: "AEV_ERR_CAPACITY",
+    -4: "AEV_ERR_STATE", -5: "AEV_ERR_UNSUPPORTED", -6: "AEV_ERR_CUDA",
+}
+
+EXPORTS = [
+    "aev_create", "aev_destroy", "aev_length", "aev_neighbors", "aev_forward", "aev_backward",
+    "ani_mlp_load", "ani_energy_forces", "aev_forward_backward_host", "ani_energy_forces_host",
+    "aev_export_pairs", "aev_status", "aev_launch_count", "aev_probe_fp32_tflops",
+    "aev_error_string",
+]
+
+
+class AevError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = lib().aev_error_string(code).decode() if _lib is not None else ""
+        super().__init__("%s failed: %s (%d) %s" % (where, ERRORS.get(code, "?"), code, msg))
+
+
+class _Params(C.Structure):
+    _fields_ = [
+        ("num_species", C.c_int32),
+        ("rcr", C.c_float), ("rca", C.c_float),
+        ("eta_r", C.c_float), ("n_shf_r", C.c_int32), ("shf_r", C.POINTER(C.c_float)),
+        ("eta_a", C.c_float), ("zeta", C.c_float),
+        ("n_shf_a", C.c_int32), ("shf_a", C.POINTER(C.c_float)),
+        ("n_shf_z", C.c_int32), ("shf_z", C.POINTER(C.c_float)),
+        ("cos_scale", C.c_float),
+        ("max_atoms", C.c_int32), ("max_batch", C.c_int32),
+        ("max_radial_nbrs", C.c_int32), ("max_angular_nbrs", C.c_int32),
+        ("device", C.c_int32),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    """Loads the C-ABI library (building it with nvcc first if the .so is absent or stale
+    and a compiler is present).  Raises if it cannot be had: there is no fallback."""
+    global _lib
+    if _lib is None:
+        path = LIB_PATH
+        try:
+            from .build import build
+            path = build()
+        except Exception:
+            if not os.path.exists(LIB_PATH):
+                raise
+        L = C.CDLL(path)
+        vp, i32, i64, f32p, i32p = C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p
+        L.aev_create.restype = C.c_int
+        L.aev_create.argtypes = [C.POINTER(_Params), C.POINTER(vp)]
+        L.aev_destroy.restype = C.c_int
+        L.aev_destroy.argtypes = [vp]
+        L.aev_length.restype = C.c_int
+        L.aev_length.argtypes = [vp]
+        L.aev_neighbors.restype = C.c_int
+        L.aev_neighbors.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, vp]
+        L.aev_forward.restype = C.c_int
+        L.aev_forward.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, f32p, vp]
+        L.aev_backward.restype = C.c_int
+        L.aev_backward.argtypes = [vp, f32p, f32p, vp]
+        L.ani_mlp_load.restype = C.c_int
+        L.ani_mlp_load.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(C.POINTER(C.c_float)),
+                                   C.POINTER(C.POINTER(C.c_float)), C.c_float]
+        L.ani_energy_forces.restype = C.c_int
+        L.ani_energy_forces.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, vp, f32p, vp]
+        L.aev_forward_backward_host.restype = C.c_int
+        L.aev_forward_backward_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), i32, i32, vp, vp, vp]
+        L.ani_energy_forces_host.restype = C.c_int
+        L.ani_energy_forces_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), i32, i32, vp, vp]
+        L.aev_export_pairs.restype = C.c_int
+        L.aev_export_pairs.argtypes = [vp, i32, i32p, i64, C.POINTER(i64)]
+        L.aev_status.restype = C.c_int
+        L.aev_status.argtypes = [vp]
+        L.aev_launch_count.restype = i64
+        L.aev_launch_count.argtypes = [vp]
+        L.aev_probe_fp32_tflops.restype = C.c_int
+        L.aev_probe_fp32_tflops.argtypes = [i32, C.POINTER(C.c_double)]
+        L.aev_error_string.restype = C.c_char_p
+        L.aev_error_string.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != AEV_OK:
+        raise AevError(rc, where)
+
+
+def _box(box):
+    if box is None:
+        return None, None
+    arr = np.ascontiguousarray(np.asarray(box, dtype=np.float32).reshape(3))
+    return arr, arr.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+    return int(getattr(stream, "cuda_stream", stream))
+
+
+def _dev_ptr(t, dtype, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA tensor" % name)
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError("%s must be contiguous %s" % (name, dtype))
+    return t.data_ptr()
+
+
+class Context:
+    """Owns one `aev_ctx`.  `params` is any object with the fields of gen.AniParams."""
+
+    def __init__(self, params, max_atoms: int, max_batch: int = 1, device: int = 0,
+                 max_radial_nbrs: int = 0, max_angular_nbrs: int = 0):
+        self._h = C.c_void_p()
+        shf_r = np.ascontiguousarray(params.shf_r, dtype=np.float32)
+        shf_a = np.ascontiguousarray(params.shf_a, dtype=np.float32)
+        shf_z = np.ascontiguousarray(params.shf_z, dtype=np.float32)
+        fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+        p = _Params(int(params.num_species), float(params.rcr), float(params.rca),
+                    float(params.eta_r), len(shf_r), fp(shf_r),
+                    float(params.eta_a), float(params.zeta), len(shf_a), fp(shf_a),
+                    len(shf_z), fp(shf_z), float(params.cos_scale),
+                    int(max_atoms), int(max_batch), int(max_radial_nbrs), int(max_angular_nbrs),
+                    int(device))
+        _check(lib().aev_create(C.byref(p), C.byref(self._h)), "aev_create")
+        self.device = int(device)
+        self.length = int(lib().aev_length(self._h))
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().aev_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- device-pointer calls (torch CUDA tensors in, asynchronous on the current stream)
+    def aev_neighbors(self, pos, species, box=None, stream=None):
+        import torch
+        batch, n = pos.shape[0], pos.shape[1]
+        keep, bp = _box(box)
+        sp = None if species is None else _dev_ptr(species, torch.int32, "species")
+        _check(lib().aev_neighbors(self._h, _dev_ptr(pos, torch.float32, "pos"), sp, bp, n, batch,
+                                   _stream(stream)), "aev_neighbors")
+
+    def aev_forward(self, pos, species, box=None, aev_out=None, stream=None):
+        import torch
+        batch, n = pos.shape[0], pos.shape[1]
+        if aev_out is None:
+            aev_out = torch.empty((batch, n, self.length), dtype=torch.float32, device=pos.device)
+        keep, bp = _box(box)
+        _check(lib().aev_forward(self._h, _dev_ptr(pos, torch.float32, "pos"),
+                                 _dev_ptr(species, torch.int32, "species"), bp, n, batch,
+                                 _dev_ptr(aev_out, torch.float32, "aev_out"), _stream(stream)),
+               "aev_forward")
+        return aev_out
+
+    def aev_backward(self, grad_aev, forces_out=None, stream=None):
+        import torch
+        if forces_out is None:
+            forces_out = torch.empty(grad_aev.shape[:2] + (3,), dtype=torch.float32, device=grad_aev.device)
+        _check(lib().aev_backward(self._h, _dev_ptr(grad_aev, torch.float32, "grad_aev"),
+                                  _dev_ptr(forces_out, torch.float32, "forces_out"), _stream(stream)),
+               "aev_backward")
+        return forces_out
+
+    def ani_mlp_load(self, species: int, weights: Sequence[np.ndarray], biases: Sequence[np.ndarray],
+                     celu_alpha: float):
+        ws = [np.ascontiguousarray(w, dtype=np.float32) for w in weights]
+        bs = [np.ascontiguousarray(b, dtype=np.float32) for b in biases]
+        dims = (C.c_int32 * (len(ws) + 1))(*([ws[0].shape[0]] + [w.shape[1] for w in ws]))
+        fpp = C.POINTER(C.c_float)
+        wp = (fpp * len(ws))(*[w.ctypes.data_as(fpp) for w in ws])
+        bp = (fpp * len(bs))(*[b.ctypes.data_as(fpp) for b in bs])
+        _check(lib().ani_mlp_load(self._h, int(species), len(ws), dims, wp, bp, float(celu_alpha)),
+               "ani_mlp_load")
+
+    def ani_energy_forces(self, pos, species, box=None, energy_out=None, forces_out=None, stream=None):
+        import torch
+        batch, n = pos.shape[0], pos.shape[1]
+        if energy_out is None:
+            energy_out = torch.empty((batch,), dtype=torch.float64, device=pos.device)
+        if forces_out is None:
+            forces_out = torch.empty((batch, n, 3), dtype=torch.float32, device=pos.device)
+        keep, bp = _box(box)
+        _check(lib().ani_energy_forces(self._h, _dev_ptr(pos, torch.float32, "pos"),
+                                       _dev_ptr(species, torch.int32, "species"), bp, n, batch,
+                                       _dev_ptr(energy_out, torch.float64, "energy_out"),
+                                       _dev_ptr(forces_out, torch.float32, "forces_out"),
+                                       _stream(stream)), "ani_energy_forces")
+        return energy_out, forces_out
+
+    # -- host-buffer calls (numpy in / out; synchronous)
+    def aev_forward_backward_host(self, pos: np.ndarray, species: np.ndarray, box, grad_aev: Optional[np.ndarray],
+                                  aev_out: Optional[np.ndarray] = None, forces_out: Optional[np.ndarray] = None):
+        batch, n = pos.shape[0], pos.shape[1]
+        assert pos.dtype == np.float32 and pos.flags.c_contiguous
+        assert species.dtype == np.int32 and species.flags.c_contiguous
+        keep, bp = _box(box)
+        if aev_out is None:
+            aev_out = np.empty((batch, n, self.length), dtype=np.float32)
+        gp = None
+        if grad_aev is not None:
+            assert grad_aev.dtype == np.float32 and grad_aev.flags.c_contiguous
+            gp = grad_aev.ctypes.data
+            if forces_out is None:
+                forces_out = np.empty((batch, n, 3), dtype=np.float32)
+        _check(lib().aev_forward_backward_host(self._h, pos.ctypes.data, species.ctypes.data, bp, n, batch,
+                                               gp, aev_out.ctypes.data,
+                                               None if forces_out is None else forces_out.ctypes.data),
+               "aev_forward_backward_host")
+        return aev_out, forces_out
+
+    def ani_energy_forces_host(self, pos: np.ndarray, species: np.ndarray, box):
+        batch, n = pos.shape[0], pos.shape[1]
+        assert pos.dtype == np.float32 and pos.flags.c_contiguous
+        assert species.dtype == np.int32 and species.flags.c_contiguous
+        keep, bp = _box(box)
+        energy = np.empty((batch,), dtype=np.float64)
+        forces = np.empty((batch, n, 3), dtype=np.float32)
+        _check(lib().ani_energy_forces_host(self._h, pos.ctypes.data, species.ctypes.data, bp, n, batch,
+                                            energy.ctypes.data, forces.ctypes.data),
+               "ani_energy_forces_host")
+        return energy, forces
+
+    # -- diagnostics
+    def aev_export_pairs(self, which: int, cap: int):
+        """Returns the (i<j) pairs of the last neighbour build as a sorted int32 [count,2] array."""
+        import torch
+        out = torch.empty((max(cap, 1), 2), dtype=torch.int32, device="cuda:%d" % self.device)
+        cnt = C.c_int64(0)
+        _check(lib().aev_export_pairs(self._h, int(which), out.data_ptr(), int(cap), C.byref(cnt)),
+               "aev_export_pairs")
+        if cnt.value > cap:
+            return self.aev_export_pairs(which, int(cnt.value))
+        arr = out[: cnt.value].cpu().numpy()
+        order = np.lexsort((arr[:, 1], arr[:, 0]))
+        return arr[order]
+
+    def aev_status(self) -> int:
+        return int(lib().aev_status(self._h))
+
+    def check_status(self):
+        _check(self.aev_status(), "aev_status")
+
+    def launch_count(self) -> int:
+        return int(lib().aev_launch_count(self._h))
+
+
+def probe_fp32_tflops(device: int = 0) -> float:
+    out = C.c_double(0.0)
+    _check(lib().aev_probe_fp32_tflops(int(device), C.byref(out)), "aev_probe_fp32_tflops")
+    return float(out.value)

@@ -1,0 +1,123 @@
+// aev_common.cuh -- context, device-side parameter block and small helpers shared by the
+// translation units of libaev_b200.so (aev_kernels.cu, ani_mlp.cu).  Product code: shares
+// nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/aev.h"
+
+namespace aevb {
+
+constexpr int kNR = 16;        // radial shifts   (BASELINE.json:configs[0])
+constexpr int kNA = 4;         // angular radial shifts
+constexpr int kNZ = 8;         // angular angle shifts
+constexpr int kBlk = kNA * kNZ;  // 32 entries per species-pair block
+constexpr int kMaxS = 8;
+constexpr int kSpeciesShift = 26;  // neighbour entry .w = j_sorted | species << 26
+constexpr int kIdxMask = (1 << kSpeciesShift) - 1;
+constexpr int kMaxMlpLayers = 4;
+
+// Everything the kernels need about the symmetry functions; passed by value (constant bank).
+struct DevParams {
+    int S, L, rad_len, n_blocks, zeta_log2;
+    float rcr, rca, rcr2, rca2;
+    float eta_r, eta_a;          // natural units (for derivatives)
+    float eta_r_l2, eta_a_l2;    // eta * log2(e)    (for ex2)
+    float inv_rcr, inv_rca;      // 1/R  (cutoff function argument r/R, used with cospi/sinpi)
+    float zeta_half;             // zeta / 2
+    float c, c2, one_m_c2;       // cos_scale, its square, 1 - c^2
+    float shf_r[kNR];
+    float shf_a[kNA];
+    float cz[kNZ], sz[kNZ];      // cos / sin of the angle shifts
+};
+
+// Geometry of one call (filled on the host per call, passed by value).
+struct Geom {
+    int n_atoms, batch, n_total;
+    int periodic;
+    int ncx, ncy, ncz, ncell;    // cells per system (non-periodic: 1,1,1,1)
+    int nbins;                   // batch*ncell*S
+    int bin_cap;                 // capacity of one (cell,species) member list
+    int cap_r, cap_a;            // per-atom neighbour capacities (total radial / angular)
+    int cand_cap;                // shared-memory candidate tile capacity (float4 entries)
+    float box[3], inv_box[3], cell_scale[3];   // cell_scale = nc / L
+};
+
+// Device workspace owned by the context.
+struct Workspace {
+    float4 *wpos;        // [n_total] wrapped position + species bits (caller order)
+    int *bin_of;         // [n_total] bin id of each atom or -1
+    int *bin_cnt;        // [nbins_cap] member counts (zero between calls)
+    int *members;        // [nbins_cap*bin_cap] caller index of bin members
+    int *bin_start;      // [nbins_cap+1] exclusive scan of bin_cnt
+    float4 *spos;        // [n_total] sorted positions, .w = caller index bits
+    int *perm;           // [n_total] sorted -> caller flat index
+    float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, j|s<<26), angular first
+    int *nidx;           // [n_total][cap_a] sorted index of angular neighbour q, -1 beyond nA
+    int2 *ncount;        // [n_total] (nA, nB)
+    float4 *fang;        // [n_total][cap_a] force on angular neighbour q from centre i
+    float4 *fown;        // [n_total] force on the centre from its own terms
+    int *err;            // device error flags (bitmask)
+    unsigned long long *pair_count;  // export counter
+};
+
+struct MlpNet {
+    int loaded;
+    int n_layers;
+    int dims[kMaxMlpLayers + 1];
+    void *w_hi[kMaxMlpLayers];   // bf16 [out][in] (K-major), hi part
+    void *w_lo[kMaxMlpLayers];   // bf16 [out][in], lo part
+    float *w_f32[kMaxMlpLayers]; // f32 [in][out] as given
+    float *w_t[kMaxMlpLayers];   // f32 [out][in] (transposed copy for the backward chain)
+    float *bias[kMaxMlpLayers];  // f32 [out]
+};
+
+}  // namespace aevb
+
+struct aev_ctx {
+    aev_params hp;               // host copy of the parameters (pointers nulled)
+    aevb::DevParams dp;
+    aevb::Geom geom;             // geometry of the most recent neighbour build
+    aevb::Workspace ws;
+    int device;
+    int sm_count;
+    int state;                   // 0 none, 1 neighbours built, 2 forward done
+    int64_t launches;
+    cudaStream_t last_stream;
+    size_t cap_total;            // atoms the workspace is sized for
+    size_t nbins_cap, members_cap;
+    int fwd_smem_optin;          // bytes of dynamic smem the forward kernel was opted into
+    // MLP
+    aevb::MlpNet nets[aevb::kMaxS];
+    float celu_alpha;
+    size_t mlp_cap;              // atoms the MLP workspaces are sized for
+    float *mlp_aev;              // [n_total][L]   (ani_energy_forces workspace)
+    float *mlp_grad;             // [n_total][L]
+    void *mlp_work;              // MLP scratch (activations)
+    size_t mlp_work_bytes;
+    int *sp_rows;                // [S][n_total] caller indices grouped by species
+    int *sp_count;               // [S]
+    // host staging (pinned) + device staging for the *_host entry points
+    void *h_pin; size_t h_pin_bytes;
+    void *d_stage; size_t d_stage_bytes;
+};
+
+namespace aevb {
+
+#define AEVB_CUDA(call)                                   \
+    do {                                                  \
+        cudaError_t e__ = (call);                         \
+        if (e__ != cudaSuccess) return AEV_ERR_CUDA;      \
+    } while (0)
+
+enum { kErrBitCapacity = 1, kErrBitState = 2 };
+
+// MLP entry points implemented in ani_mlp.cu
+int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_atoms, int batch,
+                         const float *aev, float *grad_aev, double *energy_out,
+                         cudaStream_t st);
+void mlp_free(aev_ctx *c);
+
+}  // namespace aevb

@@ -1,0 +1,294 @@
+// ani_mlp.cu -- species-batched per-atom networks:
+//   z^l = h^(l-1) W^l + b^l,  h^l = CELU_alpha(z^l) (hidden), last layer linear, E = sum_i E_i,
+//   and the transposed chain dE/dAEV (BASELINE.json:configs[4]; DESIGN.md section 3 step 6).
+#include <cuda_bf16.h>
+#include <math.h>
+#include <string.h>
+
+#include <vector>
+
+#include "aev_common.cuh"
+
+using namespace aevb;
+
+namespace {
+
+struct MlpDev {
+    int loaded, n_layers;
+    int dims[kMaxMlpLayers + 1];
+    const float *w[kMaxMlpLayers];
+    const float *wt[kMaxMlpLayers];
+    const float *b[kMaxMlpLayers];
+};
+struct MlpAll { MlpDev net[kMaxS]; };
+
+// Stable partition of the caller's atoms by species: sp_rows[s][0..sp_count[s]) in increasing
+// caller index.  One CTA; each thread owns a contiguous slice.
+__global__ void __launch_bounds__(1024) k_group(int n_total, int S, const int32_t *__restrict__ species,
+                                                int *__restrict__ sp_rows, int *__restrict__ sp_count,
+                                                double *__restrict__ energy, int batch)
+{
+    __shared__ int s_warp[32];
+    __shared__ int s_tot;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int b = tid; b < batch; b += 1024) energy[b] = 0.0;
+    const int per = (n_total + 1023) / 1024;
+    const int beg = min(tid * per, n_total), end = min(beg + per, n_total);
+    for (int s = 0; s < S; ++s) {
+        int local = 0;
+        for (int a = beg; a < end; ++a) local += (species[a] == s);
+        int incl = local;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) s_warp[wid] = incl;
+        __syncthreads();
+        if (wid == 0) {
+            int v = s_warp[lane], iv = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int u = __shfl_up_sync(0xffffffffu, iv, o);
+                if (lane >= o) iv += u;
+            }
+            s_warp[lane] = iv - v;
+            if (lane == 31) s_tot = iv;
+        }
+        __syncthreads();
+        int run = s_warp[wid] + incl - local;
+        for (int a = beg; a < end; ++a)
+            if (species[a] == s) sp_rows[(size_t)s * n_total + run++] = a;
+        if (tid == 0) sp_count[s] = s_tot;
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ float celu_f(float x, float alpha, float inv_alpha)
+{
+    return x > 0.f ? x : alpha * (__expf(x * inv_alpha) - 1.0f);
+}
+// CELU'(z) expressed through h = CELU(z): 1 for h > 0, else exp(z/alpha) = h/alpha + 1
+__device__ __forceinline__ float dcelu_from_h(float h, float inv_alpha)
+{
+    return h > 0.f ? 1.0f : fmaf(h, inv_alpha, 1.0f);
+}
+
+// v0: fp32 CUDA-core evaluation, TM rows per CTA, activations in shared memory.
+template <int TM>
+__global__ void __launch_bounds__(256)
+k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_rows,
+          const int *__restrict__ sp_count, const float *__restrict__ aev, float *__restrict__ grad,
+          double *__restrict__ energy, float alpha, int *__restrict__ err)
+{
+    extern __shared__ __align__(16) float sm[];
+    const int s = blockIdx.y;
+    const int rows = sp_count[s];
+    const int r0 = blockIdx.x * TM;
+    if (r0 >= rows) return;
+    const MlpDev &N = M.net[s];
+    if (!N.loaded) { if (threadIdx.x == 0) atomicOr(err, kErrBitState); return; }
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int nrow = min(TM, rows - r0);
+    const float inv_alpha = 1.0f / alpha;
+    const int nl = N.n_layers;
+    __shared__ int s_row[TM];
+    if (tid < TM) s_row[tid] = tid < nrow ? sp_rows[(size_t)s * n_total + r0 + tid] : -1;
+    __syncthreads();
+
+    // activation buffers: h[0] = AEV rows, h[l] for hidden layers
+    float *h[kMaxMlpLayers + 1];
+    {
+        float *p = sm;
+        for (int l = 0; l < nl; ++l) { h[l] = p; p += TM * N.dims[l]; }
+        h[nl] = p;
+    }
+    for (int t = tid; t < TM * (L / 4); t += 256) {
+        const int r = t / (L / 4), c4 = t - r * (L / 4);
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (s_row[r] >= 0) v = reinterpret_cast<const float4 *>(aev + (size_t)s_row[r] * L)[c4];
+        reinterpret_cast<float4 *>(h[0] + r * L)[c4] = v;
+    }
+    __syncthreads();
+
+    // forward, hidden layers
+    for (int l = 0; l < nl - 1; ++l) {
+        const int K = N.dims[l], No = N.dims[l + 1];
+        const float *W = N.w[l];
+        for (int o = tid; o < No; o += 256) {
+            float acc[TM];
+            const float bb = N.b[l][o];
+#pragma unroll
+            for (int r = 0; r < TM; ++r) acc[r] = bb;
+            for (int k = 0; k < K; k += 4) {
+                const float w0 = W[(size_t)k * No + o], w1 = W[(size_t)(k + 1) * No + o];
+                const float w2 = W[(size_t)(k + 2) * No + o], w3 = W[(size_t)(k + 3) * No + o];
+#pragma unroll
+                for (int r = 0; r < TM; ++r) {
+                    const float4 x = *reinterpret_cast<const float4 *>(h[l] + r * K + k);
+                    acc[r] = fmaf(x.x, w0, acc[r]); acc[r] = fmaf(x.y, w1, acc[r]);
+                    acc[r] = fmaf(x.z, w2, acc[r]); acc[r] = fmaf(x.w, w3, acc[r]);
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < TM; ++r) h[l + 1][r * No + o] = celu_f(acc[r], alpha, inv_alpha);
+        }
+        __syncthreads();
+    }
+    // last layer (one output): warp per row; energy summed in fp64
+    {
+        const int K = N.dims[nl - 1];
+        const float *W = N.w[nl - 1];
+        for (int r = wid; r < nrow; r += 8) {
+            float acc = 0.f;
+            for (int k = lane; k < K; k += 32) acc = fmaf(h[nl - 1][r * K + k], W[k], acc);
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            if (lane == 0) atomicAdd(&energy[s_row[r] / n_atoms], (double)(acc + N.b[nl - 1][0]));
+        }
+    }
+    // backward: d[nl-1][r][k] = W_last[k] * celu'(h[nl-1][r][k]), in place
+    {
+        const int K = N.dims[nl - 1];
+        const float *W = N.w[nl - 1];
+        for (int t = tid; t < TM * K; t += 256) {
+            const int k = t % K;
+            h[nl - 1][t] = W[k] * dcelu_from_h(h[nl - 1][t], inv_alpha);
+        }
+        __syncthreads();
+    }
+    for (int l = nl - 2; l >= 0; --l) {
+        // d_in[r][k] = sum_o W^l[k][o] d_out[r][o]   (times celu'(h[l]) unless l == 0)
+        const int K = N.dims[l], No = N.dims[l + 1];
+        const float *WT = N.wt[l];       // [No][K]
+        const float *dout = h[l + 1];
+        for (int k = tid; k < K; k += 256) {
+            float acc[TM];
+#pragma unroll
+            for (int r = 0; r < TM; ++r) acc[r] = 0.f;
+            for (int o = 0; o < No; o += 4) {
+                const float w0 = WT[(size_t)o * K + k], w1 = WT[(size_t)(o + 1) * K + k];
+                const float w2 = WT[(size_t)(o + 2) * K + k], w3 = WT[(size_t)(o + 3) * K + k];
+#pragma unroll
+                for (int r = 0; r < TM; ++r) {
+                    const float4 d = *reinterpret_cast<const float4 *>(dout + r * No + o);
+                    acc[r] = fmaf(d.x, w0, acc[r]); acc[r] = fmaf(d.y, w1, acc[r]);
+                    acc[r] = fmaf(d.z, w2, acc[r]); acc[r] = fmaf(d.w, w3, acc[r]);
+                }
+            }
+            if (l > 0) {
+#pragma unroll
+                for (int r = 0; r < TM; ++r)
+                    h[l][r * K + k] = acc[r] * dcelu_from_h(h[l][r * K + k], inv_alpha);
+            } else {
+#pragma unroll
+                for (int r = 0; r < TM; ++r)
+                    if (r < nrow) grad[(size_t)s_row[r] * L + k] = acc[r];
+            }
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace
+
+namespace aevb {
+
+void mlp_free(aev_ctx *c)
+{
+    for (int s = 0; s < kMaxS; ++s) {
+        MlpNet &n = c->nets[s];
+        for (int l = 0; l < kMaxMlpLayers; ++l) {
+            cudaFree(n.w_hi[l]); cudaFree(n.w_lo[l]); cudaFree(n.w_f32[l]); cudaFree(n.w_t[l]);
+            cudaFree(n.bias[l]);
+        }
+        memset(&n, 0, sizeof(n));
+    }
+}
+
+int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_atoms, int batch,
+                         const float *aev, float *grad_aev, double *energy_out, cudaStream_t st)
+{
+    const int S = c->dp.S, L = c->dp.L;
+    MlpAll M;
+    memset(&M, 0, sizeof(M));
+    int sum_hidden = 0;
+    for (int s = 0; s < S; ++s) {
+        const MlpNet &n = c->nets[s];
+        MlpDev &d = M.net[s];
+        d.loaded = n.loaded; d.n_layers = n.n_layers;
+        int sh = 0;
+        for (int l = 0; l <= n.n_layers; ++l) d.dims[l] = n.dims[l];
+        for (int l = 0; l < n.n_layers; ++l) {
+            d.w[l] = n.w_f32[l]; d.wt[l] = n.w_t[l]; d.b[l] = n.bias[l];
+            sh += n.dims[l];
+        }
+        if (sh > sum_hidden) sum_hidden = sh;
+    }
+    constexpr int TM = 8;
+    const size_t smem = (size_t)TM * sum_hidden * sizeof(float);
+    static size_t optin = 0;
+    if (smem > optin) {
+        AEVB_CUDA(cudaFuncSetAttribute(k_mlp_f32<TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        optin = smem;
+    }
+    k_group<<<1, 1024, 0, st>>>(n_total, S, species, c->sp_rows, c->sp_count, energy_out, batch);
+    dim3 grid((n_total + TM - 1) / TM, S);
+    k_mlp_f32<TM><<<grid, 256, smem, st>>>(M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
+                                            energy_out, c->celu_alpha, c->ws.err);
+    c->launches += 2;
+    if (cudaGetLastError() != cudaSuccess) return AEV_ERR_CUDA;
+    return AEV_OK;
+}
+
+}  // namespace aevb
+
+extern "C" int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const int32_t *dims,
+                            const float *const *weights, const float *const *biases, float celu_alpha)
+{
+    if (!c || !dims || !weights || !biases) return AEV_ERR_INVALID_ARG;
+    if (species < 0 || species >= c->dp.S) return AEV_ERR_INVALID_ARG;
+    if (n_layers < 2 || n_layers > kMaxMlpLayers) return AEV_ERR_UNSUPPORTED;
+    if (dims[0] != c->dp.L || dims[n_layers] != 1) return AEV_ERR_INVALID_ARG;
+    if (!(celu_alpha > 0.f)) return AEV_ERR_INVALID_ARG;
+    for (int l = 1; l < n_layers; ++l)
+        if (dims[l] < 16 || dims[l] > 256 || dims[l] % 16) return AEV_ERR_UNSUPPORTED;
+    for (int l = 0; l < n_layers; ++l)
+        if (!weights[l] || !biases[l]) return AEV_ERR_INVALID_ARG;
+    AEVB_CUDA(cudaSetDevice(c->device));
+    AEVB_CUDA(cudaDeviceSynchronize());
+    MlpNet &n = c->nets[species];
+    for (int l = 0; l < kMaxMlpLayers; ++l) {
+        cudaFree(n.w_hi[l]); cudaFree(n.w_lo[l]); cudaFree(n.w_f32[l]); cudaFree(n.w_t[l]); cudaFree(n.bias[l]);
+    }
+    memset(&n, 0, sizeof(n));
+    n.n_layers = n_layers;
+    for (int l = 0; l <= n_layers; ++l) n.dims[l] = dims[l];
+    for (int l = 0; l < n_layers; ++l) {
+        const int K = dims[l], No = dims[l + 1];
+        const size_t cnt = (size_t)K * No;
+        std::vector<float> wt(cnt);
+        std::vector<__nv_bfloat16> hi(cnt), lo(cnt);
+        for (int k = 0; k < K; ++k)
+            for (int o = 0; o < No; ++o) {
+                const float w = weights[l][(size_t)k * No + o];
+                wt[(size_t)o * K + k] = w;
+                const __nv_bfloat16 wh = __float2bfloat16_rn(w);
+                hi[(size_t)o * K + k] = wh;
+                lo[(size_t)o * K + k] = __float2bfloat16_rn(w - __bfloat162float(wh));
+            }
+        AEVB_CUDA(cudaMalloc((void **)&n.w_f32[l], cnt * 4));
+        AEVB_CUDA(cudaMalloc((void **)&n.w_t[l], cnt * 4));
+        AEVB_CUDA(cudaMalloc(&n.w_hi[l], cnt * 2));
+        AEVB_CUDA(cudaMalloc(&n.w_lo[l], cnt * 2));
+        AEVB_CUDA(cudaMalloc((void **)&n.bias[l], (size_t)No * 4));
+        AEVB_CUDA(cudaMemcpy(n.w_f32[l], weights[l], cnt * 4, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.w_t[l], wt.data(), cnt * 4, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.w_hi[l], hi.data(), cnt * 2, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.w_lo[l], lo.data(), cnt * 2, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.bias[l], biases[l], (size_t)No * 4, cudaMemcpyHostToDevice));
+    }
+    n.loaded = 1;
+    c->celu_alpha = celu_alpha;
+    return AEV_OK;
+}

@@ -1,0 +1,233 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle on the same
+seeded inputs (BASELINE.json:north_star tolerances, written out below).
+
+  neighbour pair sets ........ bit-exact (sorted (i<j) arrays equal)
+  AEV ........................ max-abs error <= 1e-5 * max|AEV|
+  forces (fp32) .............. relative RMS error <= 1e-4
+  C5 energy+forces ........... forces relative RMS <= 1e-3 (bf16-split GEMMs, fp32 accumulate)
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from gen import ani1x_style_params, make_c5_weights, make_workload
+from gen.workloads import CELU_ALPHA
+
+pytestmark = pytest.mark.gpu
+
+AEV_TOL = 1e-5       # max-abs relative to max|AEV|          (north_star)
+FORCE_TOL = 1e-4     # relative RMS, fp32                     (north_star)
+C5_FORCE_TOL = 1e-3  # relative RMS with bf16 GEMMs           (BASELINE.json:configs[4])
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2310_03121_b200 as p
+    return p
+
+
+def _dev(w):
+    pos = torch.from_numpy(w.pos).cuda()
+    sp = torch.from_numpy(w.species).cuda()
+    g = torch.from_numpy(w.grad_aev).cuda()
+    return pos, sp, g
+
+
+def _rel_rms(a, b):
+    return float(np.sqrt(((a - b) ** 2).sum() / (b ** 2).sum()))
+
+
+def _oracle_pairs(w, rc):
+    uc = "cell" if (w.box is not None and w.n_atoms > 6000) else "brute"
+    out = []
+    for b in range(w.batch):
+        p = oracle.pairs(w.pos[b], w.species[b], w.box, rc, uc)
+        out.append(p.astype(np.int64) + b * w.n_atoms)
+    return np.concatenate(out).astype(np.int32)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4"])
+def test_pair_sets_bit_exact(pkg, name):
+    w = make_workload(name)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch)
+    pos, sp, _ = _dev(w)
+    ctx.aev_neighbors(pos, sp, w.box)
+    ctx.check_status()
+    for which, rc in ((0, w.params.rcr), (1, w.params.rca)):
+        got = ctx.aev_export_pairs(which, cap=w.batch * w.n_atoms * 40)
+        want = _oracle_pairs(w, float(rc))
+        assert got.shape == want.shape, (name, which, got.shape, want.shape)
+        np.testing.assert_array_equal(got, want)
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,cos_scale", [("C1", 1.0), ("C1", 0.95), ("C2", 1.0), ("C2", 0.95),
+                                            ("C3", 1.0), ("C3", 0.95), ("C4", 1.0)])
+def test_aev_and_forces_match_oracle(pkg, name, cos_scale):
+    w = make_workload(name, cos_scale)
+    uc = w.box is not None
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch)
+    pos, sp, g = _dev(w)
+    aev = ctx.aev_forward(pos, sp, w.box)
+    forces = ctx.aev_backward(g)
+    ctx.check_status()
+    aev = aev.cpu().numpy().astype(np.float64)
+    forces = forces.cpu().numpy().astype(np.float64)
+    want_aev = oracle.aev_forward(w.params, w.pos, w.species, w.box, use_cells=uc)
+    want_f = oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=uc)
+    err = np.abs(aev - want_aev).max() / np.abs(want_aev).max()
+    assert err <= AEV_TOL, (name, cos_scale, err)
+    rms = _rel_rms(forces, want_f)
+    assert rms <= FORCE_TOL, (name, cos_scale, rms)
+    # zero net force per system (north_star), relative to the force scale
+    net = np.abs(forces.sum(axis=1)).max()
+    assert net <= 1e-3 * np.sqrt((forces ** 2).mean()) * np.sqrt(w.n_atoms), net
+    ctx.close()
+
+
+def test_backward_is_run_to_run_identical(pkg):
+    w = make_workload("C3")
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
+    pos, sp, g = _dev(w)
+    a1 = ctx.aev_forward(pos, sp, w.box).clone()
+    f1 = ctx.aev_backward(g).clone()
+    a2 = ctx.aev_forward(pos, sp, w.box)
+    f2 = ctx.aev_backward(g)
+    ctx.check_status()
+    assert torch.equal(a1, a2)
+    assert torch.equal(f1, f2)
+    ctx.close()
+
+
+def test_atoms_outside_the_box_and_permutation(pkg):
+    """Periodic images and atom order do not change the AEV (rows permute)."""
+    w = make_workload("C3")
+    rng = np.random.default_rng(7)
+    shift = rng.integers(-2, 3, size=(w.n_atoms, 3)).astype(np.float32) * w.box[None, :]
+    pos2 = (w.pos[0] + shift).astype(np.float32)
+    perm = rng.permutation(w.n_atoms)
+    pos2, sp2 = pos2[perm][None], w.species[0][perm][None]
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
+    a1 = ctx.aev_forward(torch.from_numpy(w.pos).cuda(), torch.from_numpy(w.species).cuda(), w.box).cpu().numpy()
+    a2 = ctx.aev_forward(torch.from_numpy(pos2).cuda(), torch.from_numpy(sp2).cuda(), w.box).cpu().numpy()
+    ctx.check_status()
+    # float32 image shifts of up to 2 box lengths perturb coordinates by ~1e-5 A
+    assert np.abs(a2[0] - a1[0][perm]).max() <= 2e-3 * np.abs(a1).max()
+    want = oracle.aev_forward(w.params, pos2, sp2, w.box, use_cells=True)
+    assert np.abs(a2 - want).max() <= AEV_TOL * np.abs(want).max()
+    ctx.close()
+
+
+def test_padding_atoms_and_tiny_systems(pkg):
+    p = ani1x_style_params()
+    w = make_workload("C1")
+    # two copies of C1, the second padded with 8 extra species -1 atoms placed on top of real ones
+    n = w.n_atoms + 8
+    pos = np.zeros((2, n, 3), dtype=np.float32)
+    sp = -np.ones((2, n), dtype=np.int32)
+    pos[0, :24], sp[0, :24] = w.pos[0], w.species[0]
+    pos[1, 8:], sp[1, 8:] = w.pos[0], w.species[0]
+    pos[1, :8] = w.pos[0, :8] + 0.3
+    g = np.random.default_rng(0).standard_normal((2, n, p.aev_length)).astype(np.float32)
+    ctx = pkg.Context(p, max_atoms=n, max_batch=2)
+    aev = ctx.aev_forward(torch.from_numpy(pos).cuda(), torch.from_numpy(sp).cuda(), None)
+    f = ctx.aev_backward(torch.from_numpy(g).cuda())
+    ctx.check_status()
+    aev, f = aev.cpu().numpy(), f.cpu().numpy()
+    want = oracle.aev_forward(p, pos, sp, None)
+    want_f = oracle.aev_backward(p, pos, sp, None, g)
+    assert np.abs(aev - want).max() <= AEV_TOL * np.abs(want).max()
+    assert _rel_rms(f, want_f) <= FORCE_TOL
+    assert np.all(aev[0, 24:] == 0) and np.all(aev[1, :8] == 0)
+    assert np.all(f[0, 24:] == 0) and np.all(f[1, :8] == 0)
+    # one atom, two atoms: empty / single-pair environments
+    for m in (1, 2):
+        pos1 = np.array([[[0, 0, 0], [1.0, 0, 0]][:m]], dtype=np.float32)
+        sp1 = np.zeros((1, m), dtype=np.int32)
+        a = ctx.aev_forward(torch.from_numpy(pos1).cuda(), torch.from_numpy(sp1).cuda(), None)
+        ff = ctx.aev_backward(torch.ones_like(a))
+        ctx.check_status()
+        wa = oracle.aev_forward(p, pos1, sp1, None)
+        wf = oracle.aev_backward(p, pos1, sp1, None, np.ones_like(wa, dtype=np.float32))
+        assert np.abs(a.cpu().numpy() - wa).max() <= 1e-6
+        assert np.abs(ff.cpu().numpy() - wf).max() <= 1e-5
+    ctx.close()
+
+
+def test_golden_one_water(pkg, golden):
+    """The closed-form pin of SURVEY.md 8(c) (tests/golden/one_water_c100.txt) through the GPU path."""
+    import math
+    gold = golden("one_water_c100.txt")
+    a = math.radians(52.26)
+    pos = np.array([[[0, 0, 0], [0.9572 * math.sin(a), 0, 0.9572 * math.cos(a)],
+                     [-0.9572 * math.sin(a), 0, 0.9572 * math.cos(a)]]], dtype=np.float32)
+    sp = np.array([[3, 0, 0]], dtype=np.int32)
+    p = ani1x_style_params()
+    ctx = pkg.Context(p, max_atoms=3)
+    aev = ctx.aev_forward(torch.from_numpy(pos).cuda(), torch.from_numpy(sp).cuda(), None)
+    f = ctx.aev_backward(torch.ones_like(aev)).cpu().numpy()
+    aev = aev.cpu().numpy()
+    assert aev.sum() == pytest.approx(gold["energy_g1"][0], rel=2e-6)
+    np.testing.assert_allclose(aev[0, 0, 64:72], gold["centreO_HH_row0"], rtol=2e-5, atol=1e-9)
+    np.testing.assert_allclose(aev[0, 1, 64 + 3 * 32:64 + 3 * 32 + 8], gold["centreH1_HO_row0"], rtol=2e-5, atol=1e-9)
+    for row, key in enumerate(("grad_O", "grad_H1", "grad_H2")):       # forces = -grad
+        np.testing.assert_allclose(f[0, row], -np.array(gold[key]), rtol=2e-5, atol=2e-6)
+    ctx.close()
+
+
+def test_errors(pkg):
+    p = ani1x_style_params()
+    w = make_workload("C1")
+    ctx = pkg.Context(p, max_atoms=64, max_batch=1)
+    pos, sp, g = _dev(w)
+    with pytest.raises(pkg.AevError) as e:          # backward before forward
+        ctx.aev_backward(g)
+    assert e.value.code == -4
+    with pytest.raises(pkg.AevError) as e:          # box edge < 2*rcr
+        ctx.aev_forward(pos, sp, np.array([9.0, 20.0, 20.0], dtype=np.float32))
+    assert e.value.code == -2
+    with pytest.raises(pkg.AevError) as e:          # more atoms than the context was sized for
+        big = torch.zeros((1, 65, 3), device="cuda")
+        ctx.aev_forward(big, torch.zeros((1, 65), dtype=torch.int32, device="cuda"), None)
+    assert e.value.code == -1
+    ctx.close()
+    # capacity overflow is detected on the device and surfaced by aev_status
+    ctx = pkg.Context(p, max_atoms=24, max_radial_nbrs=16, max_angular_nbrs=4)
+    ctx.aev_forward(pos, sp, None)
+    assert ctx.aev_status() == -3
+    ctx.close()
+
+
+def test_host_entry_point_matches_device_entry_point(pkg):
+    w = make_workload("C2")
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch)
+    pos, sp, g = _dev(w)
+    a1 = ctx.aev_forward(pos, sp, None).cpu().numpy()
+    f1 = ctx.aev_backward(g).cpu().numpy()
+    a2, f2 = ctx.aev_forward_backward_host(w.pos, w.species, None, w.grad_aev)
+    np.testing.assert_array_equal(a1, a2)
+    np.testing.assert_array_equal(f1, f2)
+    ctx.close()
+
+
+def test_c5_energy_and_forces(pkg):
+    w = make_workload("C5")
+    nets = make_c5_weights()
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    pos, sp, _ = _dev(w)
+    e, f = ctx.ani_energy_forces(pos, sp, w.box)
+    ctx.check_status()
+    e, f = e.cpu().numpy(), f.cpu().numpy().astype(np.float64)
+    we, wf, _ = oracle.energy_forces(w.params, w.pos, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
+    assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    assert _rel_rms(f, wf) <= C5_FORCE_TOL
+    e2, f2 = ctx.ani_energy_forces_host(w.pos, w.species, w.box)
+    assert abs(e2[0] - e[0]) <= 1e-9 * max(1.0, abs(e[0]))
+    np.testing.assert_array_equal(f2, f.astype(np.float32))
+    ctx.close()
