@@ -167,6 +167,16 @@ int ani_energy_forces_host(aev_ctx *c, const float *pos, const int32_t *species,
  */
 int aev_export_pairs(aev_ctx *c, int32_t which, int32_t *pairs_out, int64_t cap,
                      int64_t *count_out);
+/* Per-atom neighbour counts of the last neighbour build, caller's atom order:
+ *   counts_out  device i32 [batch][n_atoms][2] = (angular-set size, radial-only size); padding
+ *   atoms get (0,0).  Asynchronous on the context's last stream. */
+int aev_export_counts(aev_ctx *c, int32_t *counts_out);
+/* Per-kernel device timing for bench.py's roofline: when enabled, every kernel launch is
+ * bracketed by CUDA events on its stream.  aev_get_profile syncs, adds the elapsed times
+ * since the last call to ms_out[0..4] = {bin, sort, forward, backward, reduce} plus
+ * ms_out[5] = MLP, writes the launches seen per slot to n_out[0..5], and resets. */
+int aev_set_profiling(aev_ctx *c, int32_t enable);
+int aev_get_profile(aev_ctx *c, double *ms_out, int64_t *n_out);
 /* Syncs the context's last stream and returns AEV_OK or the deferred device-side error
  * (AEV_ERR_CAPACITY, AEV_ERR_STATE) raised by any call since the last aev_status. */
 int aev_status(aev_ctx *c);

@@ -29,7 +29,7 @@ ERRORS = {
 EXPORTS = [
     "aev_create", "aev_destroy", "aev_length", "aev_neighbors", "aev_forward", "aev_backward",
     "ani_mlp_load", "ani_energy_forces", "aev_forward_backward_host", "ani_energy_forces_host",
-    "aev_export_pairs", "aev_status", "aev_launch_count", "aev_probe_fp32_tflops",
+    "aev_export_pairs", "aev_export_counts", "aev_set_profiling", "aev_get_profile", "aev_status", "aev_launch_count", "aev_probe_fp32_tflops",
     "aev_error_string",
 ]
 
@@ -96,6 +96,12 @@ def lib():
         L.ani_energy_forces_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), i32, i32, vp, vp]
         L.aev_export_pairs.restype = C.c_int
         L.aev_export_pairs.argtypes = [vp, i32, i32p, i64, C.POINTER(i64)]
+        L.aev_export_counts.restype = C.c_int
+        L.aev_export_counts.argtypes = [vp, i32p]
+        L.aev_set_profiling.restype = C.c_int
+        L.aev_set_profiling.argtypes = [vp, i32]
+        L.aev_get_profile.restype = C.c_int
+        L.aev_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
         L.aev_status.restype = C.c_int
         L.aev_status.argtypes = [vp]
         L.aev_launch_count.restype = i64
@@ -270,6 +276,24 @@ class Context:
         arr = out[: cnt.value].cpu().numpy()
         order = np.lexsort((arr[:, 1], arr[:, 0]))
         return arr[order]
+
+    def aev_export_counts(self, batch: int, n_atoms: int):
+        """(angular, radial-only) neighbour counts per atom, int32 [batch, n_atoms, 2] on the device."""
+        import torch
+        out = torch.empty((batch, n_atoms, 2), dtype=torch.int32, device="cuda:%d" % self.device)
+        _check(lib().aev_export_counts(self._h, out.data_ptr()), "aev_export_counts")
+        return out
+
+    def aev_set_profiling(self, enable: bool):
+        _check(lib().aev_set_profiling(self._h, int(bool(enable))), "aev_set_profiling")
+
+    def aev_get_profile(self):
+        """{kernel: (total ms, launches)} since the last call (syncs)."""
+        ms = (C.c_double * 6)()
+        n = (C.c_int64 * 6)()
+        _check(lib().aev_get_profile(self._h, ms, n), "aev_get_profile")
+        names = ("bin", "sort", "forward", "backward", "reduce", "mlp")
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(names)}
 
     def aev_status(self) -> int:
         return int(lib().aev_status(self._h))

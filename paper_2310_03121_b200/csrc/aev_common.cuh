@@ -100,6 +100,8 @@ struct aev_ctx {
     int *sp_rows;                // [S][n_total] caller indices grouped by species
     int *sp_count;               // [S]
     // host staging (pinned) + device staging for the *_host entry points
+    int profiling;
+    void *prof;                  // std::vector<ProfRec>* (aev_kernels.cu)
     void *h_pin; size_t h_pin_bytes;
     void *d_stage; size_t d_stage_bytes;
 };
@@ -119,5 +121,8 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
                          const float *aev, float *grad_aev, double *energy_out,
                          cudaStream_t st);
 void mlp_free(aev_ctx *c);
+// profiling brackets (aev_kernels.cu): slot 0 bin, 1 sort, 2 forward, 3 backward, 4 reduce, 5 mlp
+void prof_begin(aev_ctx *c, int slot, cudaStream_t st);
+void prof_end(aev_ctx *c, cudaStream_t st);
 
 }  // namespace aevb

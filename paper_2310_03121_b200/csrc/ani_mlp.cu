@@ -232,10 +232,12 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
         AEVB_CUDA(cudaFuncSetAttribute(k_mlp_f32<TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         optin = smem;
     }
+    prof_begin(c, 5, st);
     k_group<<<1, 1024, 0, st>>>(n_total, S, species, c->sp_rows, c->sp_count, energy_out, batch);
     dim3 grid((n_total + TM - 1) / TM, S);
     k_mlp_f32<TM><<<grid, 256, smem, st>>>(M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
                                             energy_out, c->celu_alpha, c->ws.err);
+    prof_end(c, st);
     c->launches += 2;
     if (cudaGetLastError() != cudaSuccess) return AEV_ERR_CUDA;
     return AEV_OK;
