@@ -312,6 +312,13 @@ def run_ours(args):
         "work": wc,
     }
 
+    if args.quick:
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "ms_per_step": total_ms / args.steps, "quick": True, "roofline": roofline,
+                          "gpu_launches": int(launches), "clocks": clocks}))
+        ctx.close()
+        return
+
     # ---- end to end through the host-buffer entry point (pinned staging inside the library)
     e2e_steps = max(3, min(args.steps, 20))
     ctx.aev_forward_backward_host(w.pos, w.species, w.box, w.grad_aev)
@@ -392,6 +399,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--quick", action="store_true",
+                    help="headline loop + per-kernel pass only (for ncu runs): no e2e / other configs / cpu baseline")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps > 200:

@@ -147,6 +147,7 @@ k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_
             if (lane == 0) atomicAdd(&energy[s_row[r] / n_atoms], (double)(acc + N.b[nl - 1][0]));
         }
     }
+    __syncthreads();   // the backward chain below overwrites h[nl-1] in place
     // backward: d[nl-1][r][k] = W_last[k] * celu'(h[nl-1][r][k]), in place
     {
         const int K = N.dims[nl - 1];
