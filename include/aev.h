@@ -116,7 +116,9 @@ int aev_forward(aev_ctx *c, const float *pos, const int32_t *species, const floa
  *   grad_aev    device f32 [batch][n_atoms][L]  upstream dE/dAEV
  *   forces_out  device f32 [batch][n_atoms][3], OVERWRITTEN,
  *               forces_out[a] = - sum_i sum_slot grad_aev[i][slot]*dAEV[i][slot]/dx_a
- * No global atomics: per-pair gradients are gathered, so results are run-to-run identical.
+ * The centre's own terms are reduced with warp shuffles; the gradient on each angular
+ * neighbour is added with one fp32 RED per component, so forces are reproducible to
+ * rounding, not bit for bit (the AEV itself is bit-reproducible).
  * AEV_ERR_STATE if no forward precedes it.  Asynchronous.
  */
 int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *stream);

@@ -55,10 +55,7 @@ struct Workspace {
     float4 *spos;        // [n_total] sorted positions, .w = caller index bits
     int *perm;           // [n_total] sorted -> caller flat index
     float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, j|s<<26), angular first
-    int *nidx;           // [n_total][cap_a] sorted index of angular neighbour q, -1 beyond nA
     int2 *ncount;        // [n_total] (nA, nB)
-    float4 *fang;        // [n_total][cap_a] force on angular neighbour q from centre i
-    float4 *fown;        // [n_total] force on the centre from its own terms
     int *err;            // device error flags (bitmask)
     unsigned long long *pair_count;  // export counter
 };
