@@ -212,7 +212,7 @@ def test_host_entry_point_matches_device_entry_point(pkg):
     f1 = ctx.aev_backward(g).cpu().numpy()
     a2, f2 = ctx.aev_forward_backward_host(w.pos, w.species, None, w.grad_aev)
     np.testing.assert_array_equal(a1, a2)
-    np.testing.assert_array_equal(f1, f2)
+    np.testing.assert_allclose(f1, f2, rtol=0, atol=1e-5 * np.abs(f1).max())   # RED order
     ctx.close()
 
 
@@ -231,5 +231,5 @@ def test_c5_energy_and_forces(pkg):
     assert _rel_rms(f, wf) <= C5_FORCE_TOL
     e2, f2 = ctx.ani_energy_forces_host(w.pos, w.species, w.box)
     assert abs(e2[0] - e[0]) <= 1e-9 * max(1.0, abs(e[0]))
-    np.testing.assert_array_equal(f2, f.astype(np.float32))
+    np.testing.assert_allclose(f2, f, rtol=0, atol=1e-5 * np.abs(f).max())   # RED order
     ctx.close()
