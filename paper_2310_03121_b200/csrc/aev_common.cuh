@@ -56,6 +56,7 @@ struct Workspace {
     int *perm;           // [n_total] sorted -> caller flat index
     float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, j|s<<26), angular first
     int2 *ncount;        // [n_total] (nA, nB)
+    int *noff;           // [n_total][kMaxS+1] per-species list offsets: offA | offB << 16
     int *err;            // device error flags (bitmask)
     unsigned long long *pair_count;  // export counter
 };
