@@ -54,8 +54,9 @@ struct Workspace {
     int *bin_start;      // [nbins_cap+1] exclusive scan of bin_cnt
     float4 *spos;        // [n_total] sorted positions, .w = caller index bits
     int *perm;           // [n_total] sorted -> caller flat index
-    float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, j|s<<26), angular first
+    float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, caller index j | s<<26), angular first
     int2 *ncount;        // [n_total] (nA, nB)
+    int4 *hdr;           // [n_total] per sorted atom: (nA, nB, caller index, species)
     int *noff;           // [n_total][kMaxS+1] per-species list offsets: offA | offB << 16
     int *err;            // device error flags (bitmask)
     unsigned long long *pair_count;  // export counter
