@@ -66,8 +66,11 @@ struct MlpNet {
     int loaded;
     int n_layers;
     int dims[kMaxMlpLayers + 1];
-    void *w_hi[kMaxMlpLayers];   // bf16 [out][in] (K-major), hi part
-    void *w_lo[kMaxMlpLayers];   // bf16 [out][in], lo part
+    void *w_hi[kMaxMlpLayers];   // bf16 forward tensor-core operand  [in/8][out][8]   (ani_mlp_tc.cu)
+    void *w_lo[kMaxMlpLayers];   // bf16 backward tensor-core operand [out/8][in][8]
+    int bf16_exact;              // every hidden-layer weight is bf16-representable
+    int tc_ok;                   // shape + weights qualify for the tcgen05 kernel
+    float b_last;                // bias of the last (N = 1) layer
     float *w_f32[kMaxMlpLayers]; // f32 [in][out] as given
     float *w_t[kMaxMlpLayers];   // f32 [out][in] (transposed copy for the backward chain)
     float *bias[kMaxMlpLayers];  // f32 [out]
@@ -120,6 +123,10 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
                          const float *aev, float *grad_aev, double *energy_out,
                          cudaStream_t st);
 void mlp_free(aev_ctx *c);
+// tcgen05 path (ani_mlp_tc.cu)
+bool mlp_tc_eligible(const MlpNet &n, int L);
+int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *aev, float *grad_aev,
+                            double *energy_out, cudaStream_t st);
 // profiling brackets (aev_kernels.cu): slot 0 bin, 1 sort, 2 forward, 3 backward, 4 reduce, 5 mlp
 void prof_begin(aev_ctx *c, int slot, cudaStream_t st);
 void prof_end(aev_ctx *c, cudaStream_t st);

@@ -3,6 +3,7 @@
 //   and the transposed chain dE/dAEV (BASELINE.json:configs[4]; DESIGN.md section 3 step 6).
 #include <cuda_bf16.h>
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -195,6 +196,9 @@ k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_
 
 namespace aevb {
 
+void mlp_tc_pack(const float *w, int K_in, int N_out, std::vector<__nv_bfloat16> &fwd, std::vector<__nv_bfloat16> &bwd,
+                 bool *exact);
+
 void mlp_free(aev_ctx *c)
 {
     for (int s = 0; s < kMaxS; ++s) {
@@ -235,6 +239,16 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
     }
     prof_begin(c, 5, st);
     k_group<<<1, 1024, 0, st>>>(n_total, S, species, c->sp_rows, c->sp_count, energy_out, batch);
+    // tensor-core path when every loaded network qualifies (ani_mlp_tc.cu); else fp32 CUDA cores
+    bool all_tc = true;
+    for (int s = 0; s < S; ++s)
+        if (c->nets[s].loaded && !c->nets[s].tc_ok) all_tc = false;
+    if (all_tc && !getenv("AEVB_MLP_FP32")) {
+        const int rc = mlp_tc_forward_backward(c, n_total, n_atoms, aev, grad_aev, energy_out, st);
+        prof_end(c, st);
+        c->launches += 2;
+        return rc;
+    }
     dim3 grid((n_total + TM - 1) / TM, S);
     k_mlp_f32<TM><<<grid, 256, smem, st>>>(M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
                                             energy_out, c->celu_alpha, c->ws.err);
@@ -266,31 +280,31 @@ extern "C" int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const
     }
     memset(&n, 0, sizeof(n));
     n.n_layers = n_layers;
+    n.bf16_exact = 1;
     for (int l = 0; l <= n_layers; ++l) n.dims[l] = dims[l];
     for (int l = 0; l < n_layers; ++l) {
         const int K = dims[l], No = dims[l + 1];
         const size_t cnt = (size_t)K * No;
         std::vector<float> wt(cnt);
-        std::vector<__nv_bfloat16> hi(cnt), lo(cnt);
+        std::vector<__nv_bfloat16> fw, bw;
+        bool exact = true;
+        mlp_tc_pack(weights[l], K, No, fw, bw, &exact);
+        if (l < n_layers - 1 && !exact) n.bf16_exact = 0;
         for (int k = 0; k < K; ++k)
-            for (int o = 0; o < No; ++o) {
-                const float w = weights[l][(size_t)k * No + o];
-                wt[(size_t)o * K + k] = w;
-                const __nv_bfloat16 wh = __float2bfloat16_rn(w);
-                hi[(size_t)o * K + k] = wh;
-                lo[(size_t)o * K + k] = __float2bfloat16_rn(w - __bfloat162float(wh));
-            }
+            for (int o = 0; o < No; ++o) wt[(size_t)o * K + k] = weights[l][(size_t)k * No + o];
         AEVB_CUDA(cudaMalloc((void **)&n.w_f32[l], cnt * 4));
         AEVB_CUDA(cudaMalloc((void **)&n.w_t[l], cnt * 4));
-        AEVB_CUDA(cudaMalloc(&n.w_hi[l], cnt * 2));
-        AEVB_CUDA(cudaMalloc(&n.w_lo[l], cnt * 2));
+        AEVB_CUDA(cudaMalloc(&n.w_hi[l], fw.size() * 2));
+        AEVB_CUDA(cudaMalloc(&n.w_lo[l], bw.size() * 2));
         AEVB_CUDA(cudaMalloc((void **)&n.bias[l], (size_t)No * 4));
         AEVB_CUDA(cudaMemcpy(n.w_f32[l], weights[l], cnt * 4, cudaMemcpyHostToDevice));
         AEVB_CUDA(cudaMemcpy(n.w_t[l], wt.data(), cnt * 4, cudaMemcpyHostToDevice));
-        AEVB_CUDA(cudaMemcpy(n.w_hi[l], hi.data(), cnt * 2, cudaMemcpyHostToDevice));
-        AEVB_CUDA(cudaMemcpy(n.w_lo[l], lo.data(), cnt * 2, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.w_hi[l], fw.data(), fw.size() * 2, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.w_lo[l], bw.data(), bw.size() * 2, cudaMemcpyHostToDevice));
         AEVB_CUDA(cudaMemcpy(n.bias[l], biases[l], (size_t)No * 4, cudaMemcpyHostToDevice));
     }
+    n.b_last = biases[n_layers - 1][0];
+    n.tc_ok = mlp_tc_eligible(n, c->dp.L) ? 1 : 0;
     n.loaded = 1;
     c->celu_alpha = celu_alpha;
     return AEV_OK;

@@ -1,0 +1,472 @@
+// ani_mlp_tc.cu -- per-species MLP forward + transposed chain on the sm_100a tensor cores
+// (BASELINE.json:configs[4] "MLP GEMMs in bf16 with fp32 accumulate").
+//
+// One CTA = one tile of 128 atoms of one species.  Every GEMM of the chain is a tcgen05.mma
+// (M = 128 rows, N = layer width, K = 16 per instruction) whose accumulator lives in TMEM:
+//   forward  z_l  = h_(l-1) W_l            A = activations (shared memory), B = W_l  [N=out][K=in]
+//   backward d_l' = d_(l+1) W_(l+1)^T      A = upstream    (shared memory), B = W^T  [N=in][K=out]
+// Activations are fp32 values split into two bf16 operands (hi + lo, error 2^-17); the weights
+// are the model's bf16-representable values (reading G14), so each GEMM is two MMAs
+// per K step.  The pre-activations z_l stay resident in TMEM between the forward and the
+// backward sweep (CELU' is recomputed from them); bias, CELU, the last (N = 1) layer, the
+// energy sum and the bf16 split run in the epilogue, one thread per row (tcgen05.ld 32x32b).
+//
+// Operand layout in shared memory (no swizzle, K-major "core matrices" of 8 rows x 16 bytes):
+//   element (r, k) of an [R x K] operand sits at  (k/8) * R*16 + r*16 + (k%8)*2  bytes,
+//   i.e. [K/8][R][8] bf16  =>  descriptor LBO = R*16 (next 8 k), SBO = 128 (next 8 rows).
+#include <cuda_bf16.h>
+#include <math.h>
+#include <string.h>
+
+#include <vector>
+
+#include "aev_common.cuh"
+
+using namespace aevb;
+
+namespace {
+
+constexpr int kTM = 128;              // rows (atoms) per tile = MMA M
+constexpr int kKC = 64;               // K chunk of the first layer (AEV columns per stage)
+constexpr int kActBytes = 81920;      // activation operand: hi | lo, each up to [256/8... K<=160][128][8] bf16
+constexpr int kActHalf = kActBytes / 2;
+constexpr int kWBufBytes = 40960;     // one weight buffer (two of them, ping-pong)
+constexpr int kTcSmem = kActBytes + 2 * kWBufBytes + 1024;
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(void *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void proxy_fence() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// D[tmem] (+)= A[smem] * B[smem]; single thread issues on behalf of the CTA.
+__device__ __forceinline__ void umma_bf16(unsigned d_tmem, unsigned long long a_desc, unsigned long long b_desc,
+                                          unsigned idesc, unsigned accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// arrive on an mbarrier once every MMA issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(void *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(unsigned taddr, float *v)
+{
+    unsigned r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(r[k]);
+}
+
+// shared-memory matrix descriptor: no swizzle, K-major, version 1 (sm_100)
+__device__ __forceinline__ unsigned long long smem_desc(unsigned addr, unsigned lbo_bytes, unsigned sbo_bytes)
+{
+    return (unsigned long long)((addr >> 4) & 0x3FFF) | ((unsigned long long)((lbo_bytes >> 4) & 0x3FFF) << 16) |
+           ((unsigned long long)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46);
+}
+// instruction descriptor: kind::f16, A = B = bf16 (K-major), D = f32, M = 128, N = n
+__device__ __forceinline__ unsigned instr_desc(int n)
+{
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((unsigned)(n >> 3) << 17) | ((unsigned)(kTM >> 4) << 24);
+}
+
+__device__ __forceinline__ void cp_async16_tc(void *smem_dst, const void *gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all_tc() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// fp32 x8 -> bf16 hi x8 (16 bytes) and bf16 lo x8 (residual)
+__device__ __forceinline__ void split8(const float *v, uint4 &hi, uint4 &lo)
+{
+    unsigned h[4], l[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const __nv_bfloat16 h0 = __float2bfloat16_rn(v[2 * k]), h1 = __float2bfloat16_rn(v[2 * k + 1]);
+        const __nv_bfloat16 l0 = __float2bfloat16_rn(v[2 * k] - __bfloat162float(h0));
+        const __nv_bfloat16 l1 = __float2bfloat16_rn(v[2 * k + 1] - __bfloat162float(h1));
+        h[k] = (unsigned)__bfloat16_as_ushort(h0) | ((unsigned)__bfloat16_as_ushort(h1) << 16);
+        l[k] = (unsigned)__bfloat16_as_ushort(l0) | ((unsigned)__bfloat16_as_ushort(l1) << 16);
+    }
+    hi = make_uint4(h[0], h[1], h[2], h[3]);
+    lo = make_uint4(l[0], l[1], l[2], l[3]);
+}
+
+__device__ __forceinline__ float celu_tc(float x, float alpha, float inv_alpha)
+{
+    return x > 0.f ? x : alpha * (__expf(x * inv_alpha) - 1.0f);
+}
+__device__ __forceinline__ float dcelu_tc(float x, float inv_alpha) { return x > 0.f ? 1.0f : __expf(x * inv_alpha); }
+
+struct TcNetDev {
+    int loaded, nh;                      // nh = hidden layers (1..3); layer l maps dims[l] -> dims[l+1]
+    int dims[kMaxMlpLayers + 1];         // dims[0] = L, dims[1..nh] hidden widths, dims[nh+1] = 1
+    const __nv_bfloat16 *wf[3];          // forward operand of layer l:  [K/8][N][8], K = dims[l],   N = dims[l+1]
+    const __nv_bfloat16 *wb[3];          // backward operand of layer l: [K/8][N][8], K = dims[l+1], N = dims[l]
+    const float *bias[3];                // bias of layer l (width dims[l+1])
+    const float *wlast;                  // last layer weights [dims[nh]]
+    float blast;
+    int zoff[3];                         // TMEM column of z_(l+1) = output of layer l
+};
+struct TcAll { TcNetDev net[kMaxS]; };
+
+__global__ void __launch_bounds__(kTM, 1)
+k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_rows,
+         const int *__restrict__ sp_count, const float *__restrict__ aev, float *__restrict__ grad,
+         double *__restrict__ energy, float alpha, int *__restrict__ err)
+{
+    extern __shared__ __align__(1024) unsigned char sm[];
+    __shared__ int s_row[kTM];
+    const int s = blockIdx.y;
+    const int rows = sp_count[s];
+    const int r0 = blockIdx.x * kTM;
+    if (r0 >= rows) return;
+    const TcNetDev &N = M.net[s];
+    if (!N.loaded) { if (threadIdx.x == 0) atomicOr(err, kErrBitState); return; }
+    const int tid = threadIdx.x, wid = tid >> 5;
+    const float inv_alpha = 1.0f / alpha;
+    const int nh = N.nh;
+
+    unsigned char *act = sm;
+    unsigned char *wbuf[2] = {sm + kActBytes, sm + kActBytes + kWBufBytes};
+    unsigned long long *bar = reinterpret_cast<unsigned long long *>(sm + kActBytes + 2 * kWBufBytes);
+    unsigned *tmem_slot = reinterpret_cast<unsigned *>(bar + 4);
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); mbar_init(&bar[2], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (wid == 0) {      // one warp owns the TMEM allocation (all 512 columns: one CTA per SM)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    s_row[tid] = (r0 + tid < rows) ? sp_rows[(size_t)s * n_total + r0 + tid] : -1;
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const unsigned tmem = *tmem_slot;
+    const unsigned tlane = tmem + ((unsigned)(wid * 32) << 16);      // this warp's quarter of the 128 lanes
+    const int my_row = s_row[tid];
+    unsigned ph0 = 0, ph1 = 0, ph2 = 0;
+
+    // ------------------------------------------------------------------ layer 0, K in chunks
+    {
+        const int K0 = N.dims[0], N1 = N.dims[1];
+        const unsigned idesc = instr_desc(N1);
+        const int nkc = (K0 + kKC - 1) / kKC;
+        for (int kc = 0; kc < nkc; ++kc) {
+            const int b = kc & 1;
+            const int kw = min(kKC, K0 - kc * kKC);
+            if (kc >= 2) {                 // the MMAs that read this buffer two chunks ago
+                if (b == 0) { mbar_wait(&bar[0], ph0); ph0 ^= 1; } else { mbar_wait(&bar[1], ph1); ph1 ^= 1; }
+            }
+            unsigned char *abuf = act + b * 32768;         // hi at +0, lo at +16384
+            unsigned char *wb_ = wbuf[b];
+            {
+                const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wf[0]) + (size_t)kc * (kKC / 8) * N1 * 16;
+                const int pieces = (kw / 8) * N1;
+                for (int t = tid; t < pieces; t += kTM) cp_async16_tc(wb_ + t * 16, src + (size_t)t * 16);
+            }
+            if (my_row >= 0) {
+                const float4 *src = reinterpret_cast<const float4 *>(aev + (size_t)my_row * L + kc * kKC);
+#pragma unroll 4
+                for (int c = 0; c < kw / 8; ++c) {
+                    const float4 x0 = src[2 * c], x1 = src[2 * c + 1];
+                    const float v[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+                    uint4 hi, lo;
+                    split8(v, hi, lo);
+                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + tid * 16) = hi;
+                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + tid * 16) = lo;
+                }
+            } else {
+                for (int c = 0; c < kw / 8; ++c) {
+                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
+                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
+                }
+            }
+            cp_async_wait_all_tc();
+            proxy_fence();
+            tc_fence_before();
+            __syncthreads();
+            if (tid == 0) {
+                tc_fence_after();
+                const unsigned a_hi = smem_u32(abuf), a_lo = a_hi + 16384, b_a = smem_u32(wb_);
+                for (int ks = 0; ks < kw / 16; ++ks) {
+                    const unsigned long long bd = smem_desc(b_a + ks * 2 * N1 * 16, N1 * 16, 128);
+                    umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 4096, 2048, 128), bd, idesc, (kc | ks) != 0);
+                    umma_bf16(tmem + N.zoff[0], smem_desc(a_lo + ks * 4096, 2048, 128), bd, idesc, 1u);
+                }
+                umma_commit(&bar[b]);
+            }
+        }
+        // drain: every outstanding commit (at most one per buffer)
+        if (nkc >= 2) {
+            mbar_wait(&bar[0], ph0); ph0 ^= 1;
+            mbar_wait(&bar[1], ph1); ph1 ^= 1;
+        } else {
+            mbar_wait(&bar[0], ph0); ph0 ^= 1;
+        }
+        tc_fence_after();
+    }
+
+    // whole-layer weight operand -> shared memory (contiguous [K/8][N][8] block)
+    auto load_w = [&](const __nv_bfloat16 *w, int K, int Nn, unsigned char *dst) {
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(w);
+        const int pieces = (K / 8) * Nn;
+        for (int t = tid; t < pieces; t += kTM) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
+    };
+    // D[tmem + dcol] = act[128 x K] (hi + lo) * B[Nn x K]^T, issued by one thread, completion on bar[2]
+    auto gemm = [&](int K, int Nn, const unsigned char *wsm, int lbo_b, unsigned dcol) {
+        if (tid == 0) {
+            tc_fence_after();
+            const unsigned a_hi = smem_u32(act), a_lo = a_hi + kActHalf, b_a = smem_u32(wsm);
+            const unsigned idesc = instr_desc(Nn);
+            for (int ks = 0; ks < K / 16; ++ks) {
+                const unsigned long long bd = smem_desc(b_a + ks * 2 * lbo_b, lbo_b, 128);
+                umma_bf16(tmem + dcol, smem_desc(a_hi + ks * 4096, 2048, 128), bd, idesc, ks != 0);
+                umma_bf16(tmem + dcol, smem_desc(a_lo + ks * 4096, 2048, 128), bd, idesc, 1u);
+            }
+            umma_commit(&bar[2]);
+        }
+    };
+    auto wait_gemm = [&]() {
+        mbar_wait(&bar[2], ph2);
+        ph2 ^= 1;
+        tc_fence_after();
+    };
+    // 16 fp32 values of this thread's row -> operand columns c0..c0+15 (hi and lo)
+    auto put16 = [&](const float *v, int c0) {
+        uint4 hi, lo;
+        split8(v, hi, lo);
+        *reinterpret_cast<uint4 *>(act + (c0 >> 3) * 2048 + tid * 16) = hi;
+        *reinterpret_cast<uint4 *>(act + kActHalf + (c0 >> 3) * 2048 + tid * 16) = lo;
+        split8(v + 8, hi, lo);
+        *reinterpret_cast<uint4 *>(act + ((c0 >> 3) + 1) * 2048 + tid * 16) = hi;
+        *reinterpret_cast<uint4 *>(act + kActHalf + ((c0 >> 3) + 1) * 2048 + tid * 16) = lo;
+    };
+    auto sync_for_mma = [&]() {      // generic-proxy writes + cp.async data visible to the tensor core
+        cp_async_wait_all_tc();
+        proxy_fence();
+        tc_fence_before();
+        __syncthreads();
+    };
+
+    // ------------------------------------------------------------------ forward, layers 1 .. nh-1
+    int wsel = 0;
+    for (int l = 1; l <= nh; ++l) {
+        // z_l (output of layer l-1) is complete in TMEM at zoff[l-1]
+        const int Nl = N.dims[l];
+        const float *bl = N.bias[l - 1];
+        if (l < nh) {
+            load_w(N.wf[l], Nl, N.dims[l + 1], wbuf[wsel]);               // overlaps the epilogue below
+            for (int c0 = 0; c0 < Nl; c0 += 16) {
+                float v[16];
+                tmem_ld16(tlane + N.zoff[l - 1] + c0, v);
+#pragma unroll
+                for (int k = 0; k < 16; ++k) v[k] = celu_tc(v[k] + __ldg(bl + c0 + k), alpha, inv_alpha);
+                put16(v, c0);
+            }
+            sync_for_mma();
+            gemm(Nl, N.dims[l + 1], wbuf[wsel], N.dims[l + 1] * 16, N.zoff[l]);
+            wsel ^= 1;
+            wait_gemm();
+        } else {
+            // last hidden layer: energy (N = 1 layer on the CUDA cores) and d_nh = w_last * CELU'(z)
+            if (nh >= 2) load_w(N.wb[nh - 1], Nl, N.dims[nh - 1], wbuf[wsel]);
+            float e = 0.f;
+            for (int c0 = 0; c0 < Nl; c0 += 16) {
+                float v[16];
+                tmem_ld16(tlane + N.zoff[l - 1] + c0, v);
+#pragma unroll
+                for (int k = 0; k < 16; ++k) {
+                    const float z = v[k] + __ldg(bl + c0 + k);
+                    const float w = __ldg(N.wlast + c0 + k);
+                    e = fmaf(celu_tc(z, alpha, inv_alpha), w, e);
+                    v[k] = w * dcelu_tc(z, inv_alpha);
+                }
+                put16(v, c0);
+            }
+            if (my_row >= 0) atomicAdd(&energy[my_row / n_atoms], (double)(e + N.blast));
+        }
+    }
+
+    // ------------------------------------------------------------------ backward, layers nh-1 .. 1
+    for (int l = nh - 1; l >= 1; --l) {
+        // act holds d_(l+1) [128 x dims[l+1]]; wbuf[wsel] holds (or is receiving) W_l^T operand
+        const int Kb = N.dims[l + 1], Nb = N.dims[l];
+        const unsigned dcol = N.zoff[l];                   // z_(l+1) is dead: reuse its columns
+        sync_for_mma();
+        gemm(Kb, Nb, wbuf[wsel], Nb * 16, dcol);
+        wsel ^= 1;
+        if (l >= 2) load_w(N.wb[l - 1], Nb, N.dims[l - 1], wbuf[wsel]);   // next operand while the MMAs run
+        wait_gemm();
+        const float *bl = N.bias[l - 1];
+        for (int c0 = 0; c0 < Nb; c0 += 16) {
+            float d[16], z[16];
+            tmem_ld16(tlane + dcol + c0, d);
+            tmem_ld16(tlane + N.zoff[l - 1] + c0, z);
+#pragma unroll
+            for (int k = 0; k < 16; ++k) d[k] *= dcelu_tc(z[k] + __ldg(bl + c0 + k), inv_alpha);
+            put16(d, c0);
+        }
+    }
+
+    // ------------------------------------------------------------------ d_0 = d_1 W_0^T, N = L in chunks of 128
+    {
+        const int Kb = N.dims[1];
+        const int nch = (L + 127) / 128;
+        auto load_chunk = [&](int j, unsigned char *dst) {
+            const int n0 = j * 128, nw = min(128, L - n0);
+            const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wb[0]);
+            const int pieces = (Kb / 8) * nw;
+            for (int t = tid; t < pieces; t += kTM) {
+                const int kc = t / nw, n = t - kc * nw;
+                cp_async16_tc(dst + t * 16, src + ((size_t)kc * L + n0 + n) * 16);
+            }
+        };
+        load_chunk(0, wbuf[wsel]);
+        sync_for_mma();
+        gemm(Kb, min(128, L), wbuf[wsel], min(128, L) * 16, 0u);
+        for (int j = 0; j < nch; ++j) {
+            const int n0 = j * 128, nw = min(128, L - n0);
+            if (j + 1 < nch) load_chunk(j + 1, wbuf[wsel ^ 1]);
+            wait_gemm();
+            if (j + 1 < nch) {
+                const int nw1 = min(128, L - (j + 1) * 128);
+                sync_for_mma();
+                gemm(Kb, nw1, wbuf[wsel ^ 1], nw1 * 16, (unsigned)((j + 1) * 128));
+                wsel ^= 1;
+            }
+            // tcgen05.ld is warp-collective: rows without an atom take part, only the store is skipped
+            float4 *dst = reinterpret_cast<float4 *>(grad + (size_t)(my_row >= 0 ? my_row : 0) * L + n0);
+            for (int c0 = 0; c0 < nw; c0 += 16) {
+                float v[16];
+                tmem_ld16(tlane + n0 + c0, v);
+                if (my_row >= 0) {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) dst[(c0 >> 2) + k] = make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+                }
+            }
+        }
+    }
+
+    // ------------------------------------------------------------------ teardown
+    tc_fence_before();
+    __syncthreads();
+    if (wid == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+}
+
+
+}  // namespace
+
+namespace aevb {
+
+// Shapes the tensor-core kernel covers (everything else runs the fp32 CUDA-core kernel):
+// 1..3 hidden layers of width 16..160 (multiples of 16), L <= 512 (multiple of 16), weight
+// operands of the inner layers <= 40 KB, z_l and the backward accumulators fit 512 TMEM columns,
+// and every hidden-layer weight is bf16-representable (the model of reading G14).
+bool mlp_tc_eligible(const MlpNet &n, int L)
+{
+    const int nh = n.n_layers - 1;
+    if (nh < 1 || nh > 3 || !n.bf16_exact) return false;
+    if (L % 16 || L > 512 || n.dims[0] != L) return false;
+    int off = 0;
+    for (int l = 1; l <= nh; ++l) {
+        if (n.dims[l] % 16 || n.dims[l] < 16 || n.dims[l] > 160) return false;
+        off += n.dims[l];
+    }
+    if (off > 512) return false;
+    if (kKC * n.dims[1] * 2 > kWBufBytes) return false;
+    for (int l = 1; l < nh; ++l)
+        if (n.dims[l] * n.dims[l + 1] * 2 > kWBufBytes) return false;
+    // backward accumulator of layer l reuses the columns from z_(l+1) on
+    int zo = 0;
+    for (int l = 1; l < nh; ++l) {
+        zo += n.dims[l];                       // = zoff of z_(l+1)
+        if (zo + n.dims[l] > 512) return false;
+    }
+    return true;
+}
+
+int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *aev, float *grad_aev,
+                            double *energy_out, cudaStream_t st)
+{
+    const int S = c->dp.S, L = c->dp.L;
+    TcAll M;
+    memset(&M, 0, sizeof(M));
+    for (int s = 0; s < S; ++s) {
+        const MlpNet &n = c->nets[s];
+        TcNetDev &d = M.net[s];
+        d.loaded = n.loaded;
+        if (!n.loaded) continue;
+        d.nh = n.n_layers - 1;
+        for (int l = 0; l <= n.n_layers; ++l) d.dims[l] = n.dims[l];
+        int off = 0;
+        for (int l = 0; l < d.nh; ++l) {
+            d.wf[l] = static_cast<const __nv_bfloat16 *>(n.w_hi[l]);
+            d.wb[l] = static_cast<const __nv_bfloat16 *>(n.w_lo[l]);
+            d.bias[l] = n.bias[l];
+            d.zoff[l] = off;
+            off += n.dims[l + 1];
+        }
+        d.wlast = n.w_f32[d.nh];
+        d.blast = n.b_last;
+    }
+    static bool optin = false;
+    if (!optin) {
+        AEVB_CUDA(cudaFuncSetAttribute(k_mlp_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmem));
+        optin = true;
+    }
+    dim3 grid((n_total + kTM - 1) / kTM, S);
+    k_mlp_tc<<<grid, kTM, kTcSmem, st>>>(M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
+                                          energy_out, c->celu_alpha, c->ws.err);
+    return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
+}
+
+// Host-side packing of one layer W[in][out] (row-major) into the two chunked operand layouts.
+void mlp_tc_pack(const float *w, int K_in, int N_out, std::vector<__nv_bfloat16> &fwd, std::vector<__nv_bfloat16> &bwd,
+                 bool *exact)
+{
+    fwd.assign((size_t)((K_in + 7) / 8) * N_out * 8, __float2bfloat16_rn(0.f));    // K padded to 8
+    bwd.assign((size_t)((N_out + 7) / 8) * K_in * 8, __float2bfloat16_rn(0.f));
+    bool ex = true;
+    for (int k = 0; k < K_in; ++k)
+        for (int o = 0; o < N_out; ++o) {
+            const float v = w[(size_t)k * N_out + o];
+            const __nv_bfloat16 b = __float2bfloat16_rn(v);
+            if (__bfloat162float(b) != v) ex = false;
+            // forward: B[n = o][kk = k]  ->  [kk/8][N_out][8]
+            fwd[((size_t)(k >> 3) * N_out + o) * 8 + (k & 7)] = b;
+            // backward: B[n = k][kk = o] ->  [kk/8][K_in][8]
+            bwd[((size_t)(o >> 3) * K_in + k) * 8 + (o & 7)] = b;
+        }
+    *exact = ex;
+}
+
+}  // namespace aevb
