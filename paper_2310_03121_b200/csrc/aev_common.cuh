@@ -101,6 +101,7 @@ struct aev_ctx {
     size_t mlp_work_bytes;
     int *sp_rows;                // [S][n_total] caller indices grouped by species
     int *sp_count;               // [S]
+    void *tc_dev;                // device copy of the tensor-core network table (ani_mlp_tc.cu)
     // host staging (pinned) + device staging for the *_host entry points
     int profiling;
     void *prof;                  // std::vector<ProfRec>* (aev_kernels.cu)
@@ -125,6 +126,7 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
 void mlp_free(aev_ctx *c);
 // tcgen05 path (ani_mlp_tc.cu)
 bool mlp_tc_eligible(const MlpNet &n, int L);
+int mlp_tc_upload(aev_ctx *c);
 int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *aev, float *grad_aev,
                             double *energy_out, cudaStream_t st);
 // profiling brackets (aev_kernels.cu): slot 0 bin, 1 sort, 2 forward, 3 backward, 4 reduce, 5 mlp

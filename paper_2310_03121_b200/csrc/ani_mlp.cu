@@ -307,5 +307,5 @@ extern "C" int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const
     n.tc_ok = mlp_tc_eligible(n, c->dp.L) ? 1 : 0;
     n.loaded = 1;
     c->celu_alpha = celu_alpha;
-    return AEV_OK;
+    return mlp_tc_upload(c);
 }

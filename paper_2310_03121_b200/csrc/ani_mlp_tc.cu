@@ -27,6 +27,8 @@ using namespace aevb;
 namespace {
 
 constexpr int kTM = 128;              // rows (atoms) per tile = MMA M
+constexpr int kTcGroups = 4;         // warpgroups per CTA: each takes every 4th block of 16 columns in the epilogues
+constexpr int kTcThreads = kTM * kTcGroups;
 constexpr int kKC = 64;               // K chunk of the first layer (AEV columns per stage)
 constexpr int kActBytes = 81920;      // activation operand: hi | lo, each up to [256/8... K<=160][128][8] bf16
 constexpr int kActHalf = kActBytes / 2;
@@ -108,11 +110,12 @@ __device__ __forceinline__ void split8(const float *v, uint4 &hi, uint4 &lo)
     unsigned h[4], l[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const __nv_bfloat16 h0 = __float2bfloat16_rn(v[2 * k]), h1 = __float2bfloat16_rn(v[2 * k + 1]);
-        const __nv_bfloat16 l0 = __float2bfloat16_rn(v[2 * k] - __bfloat162float(h0));
-        const __nv_bfloat16 l1 = __float2bfloat16_rn(v[2 * k + 1] - __bfloat162float(h1));
-        h[k] = (unsigned)__bfloat16_as_ushort(h0) | ((unsigned)__bfloat16_as_ushort(h1) << 16);
-        l[k] = (unsigned)__bfloat16_as_ushort(l0) | ((unsigned)__bfloat16_as_ushort(l1) << 16);
+        const __nv_bfloat162 hh = __floats2bfloat162_rn(v[2 * k], v[2 * k + 1]);
+        h[k] = *reinterpret_cast<const unsigned *>(&hh);
+        // bf16 -> fp32 is a 16-bit shift
+        const float f0 = __uint_as_float(h[k] << 16), f1 = __uint_as_float(h[k] & 0xffff0000u);
+        const __nv_bfloat162 ll = __floats2bfloat162_rn(v[2 * k] - f0, v[2 * k + 1] - f1);
+        l[k] = *reinterpret_cast<const unsigned *>(&ll);
     }
     hi = make_uint4(h[0], h[1], h[2], h[3]);
     lo = make_uint4(l[0], l[1], l[2], l[3]);
@@ -136,8 +139,8 @@ struct TcNetDev {
 };
 struct TcAll { TcNetDev net[kMaxS]; };
 
-__global__ void __launch_bounds__(kTM, 1)
-k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_rows,
+__global__ void __launch_bounds__(kTcThreads, 1)
+k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const int *__restrict__ sp_rows,
          const int *__restrict__ sp_count, const float *__restrict__ aev, float *__restrict__ grad,
          double *__restrict__ energy, float alpha, int *__restrict__ err)
 {
@@ -147,9 +150,13 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
     const int rows = sp_count[s];
     const int r0 = blockIdx.x * kTM;
     if (r0 >= rows) return;
-    const TcNetDev &N = M.net[s];
+    __shared__ TcNetDev N;
+    if (threadIdx.x < sizeof(TcNetDev) / 4)
+        reinterpret_cast<int *>(&N)[threadIdx.x] = reinterpret_cast<const int *>(&Mg->net[s])[threadIdx.x];
+    __syncthreads();
     if (!N.loaded) { if (threadIdx.x == 0) atomicOr(err, kErrBitState); return; }
     const int tid = threadIdx.x, wid = tid >> 5;
+    const int row = tid & (kTM - 1), grp = tid >> 7;     // epilogue: thread = (row, column group)
     const float inv_alpha = 1.0f / alpha;
     const int nh = N.nh;
 
@@ -166,13 +173,13 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    s_row[tid] = (r0 + tid < rows) ? sp_rows[(size_t)s * n_total + r0 + tid] : -1;
+    if (tid < kTM) s_row[tid] = (r0 + tid < rows) ? sp_rows[(size_t)s * n_total + r0 + tid] : -1;
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const unsigned tmem = *tmem_slot;
-    const unsigned tlane = tmem + ((unsigned)(wid * 32) << 16);      // this warp's quarter of the 128 lanes
-    const int my_row = s_row[tid];
+    const unsigned tlane = tmem + ((unsigned)((wid & 3) * 32) << 16);   // this warp's quarter of the 128 lanes
+    const int my_row = s_row[row];
     unsigned ph0 = 0, ph1 = 0, ph2 = 0;
 
     // ------------------------------------------------------------------ layer 0, K in chunks
@@ -191,23 +198,23 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
             {
                 const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wf[0]) + (size_t)kc * (kKC / 8) * N1 * 16;
                 const int pieces = (kw / 8) * N1;
-                for (int t = tid; t < pieces; t += kTM) cp_async16_tc(wb_ + t * 16, src + (size_t)t * 16);
+                for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(wb_ + t * 16, src + (size_t)t * 16);
             }
             if (my_row >= 0) {
                 const float4 *src = reinterpret_cast<const float4 *>(aev + (size_t)my_row * L + kc * kKC);
-#pragma unroll 4
-                for (int c = 0; c < kw / 8; ++c) {
+#pragma unroll 2
+                for (int c = grp; c < kw / 8; c += kTcGroups) {
                     const float4 x0 = src[2 * c], x1 = src[2 * c + 1];
                     const float v[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
                     uint4 hi, lo;
                     split8(v, hi, lo);
-                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + tid * 16) = hi;
-                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + tid * 16) = lo;
+                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + row * 16) = hi;
+                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + row * 16) = lo;
                 }
             } else {
-                for (int c = 0; c < kw / 8; ++c) {
-                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
-                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
+                for (int c = grp; c < kw / 8; c += kTcGroups) {
+                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + row * 16) = make_uint4(0, 0, 0, 0);
+                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + row * 16) = make_uint4(0, 0, 0, 0);
                 }
             }
             cp_async_wait_all_tc();
@@ -239,7 +246,7 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
     auto load_w = [&](const __nv_bfloat16 *w, int K, int Nn, unsigned char *dst) {
         const unsigned char *src = reinterpret_cast<const unsigned char *>(w);
         const int pieces = (K / 8) * Nn;
-        for (int t = tid; t < pieces; t += kTM) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
+        for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
     };
     // D[tmem + dcol] = act[128 x K] (hi + lo) * B[Nn x K]^T, issued by one thread, completion on bar[2]
     auto gemm = [&](int K, int Nn, const unsigned char *wsm, int lbo_b, unsigned dcol) {
@@ -264,11 +271,11 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
     auto put16 = [&](const float *v, int c0) {
         uint4 hi, lo;
         split8(v, hi, lo);
-        *reinterpret_cast<uint4 *>(act + (c0 >> 3) * 2048 + tid * 16) = hi;
-        *reinterpret_cast<uint4 *>(act + kActHalf + (c0 >> 3) * 2048 + tid * 16) = lo;
+        *reinterpret_cast<uint4 *>(act + (c0 >> 3) * 2048 + row * 16) = hi;
+        *reinterpret_cast<uint4 *>(act + kActHalf + (c0 >> 3) * 2048 + row * 16) = lo;
         split8(v + 8, hi, lo);
-        *reinterpret_cast<uint4 *>(act + ((c0 >> 3) + 1) * 2048 + tid * 16) = hi;
-        *reinterpret_cast<uint4 *>(act + kActHalf + ((c0 >> 3) + 1) * 2048 + tid * 16) = lo;
+        *reinterpret_cast<uint4 *>(act + ((c0 >> 3) + 1) * 2048 + row * 16) = hi;
+        *reinterpret_cast<uint4 *>(act + kActHalf + ((c0 >> 3) + 1) * 2048 + row * 16) = lo;
     };
     auto sync_for_mma = [&]() {      // generic-proxy writes + cp.async data visible to the tensor core
         cp_async_wait_all_tc();
@@ -285,7 +292,7 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
         const float *bl = N.bias[l - 1];
         if (l < nh) {
             load_w(N.wf[l], Nl, N.dims[l + 1], wbuf[wsel]);               // overlaps the epilogue below
-            for (int c0 = 0; c0 < Nl; c0 += 16) {
+            for (int c0 = grp * 16; c0 < Nl; c0 += 16 * kTcGroups) {
                 float v[16];
                 tmem_ld16(tlane + N.zoff[l - 1] + c0, v);
 #pragma unroll
@@ -300,7 +307,7 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
             // last hidden layer: energy (N = 1 layer on the CUDA cores) and d_nh = w_last * CELU'(z)
             if (nh >= 2) load_w(N.wb[nh - 1], Nl, N.dims[nh - 1], wbuf[wsel]);
             float e = 0.f;
-            for (int c0 = 0; c0 < Nl; c0 += 16) {
+            for (int c0 = grp * 16; c0 < Nl; c0 += 16 * kTcGroups) {
                 float v[16];
                 tmem_ld16(tlane + N.zoff[l - 1] + c0, v);
 #pragma unroll
@@ -312,7 +319,7 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
                 }
                 put16(v, c0);
             }
-            if (my_row >= 0) atomicAdd(&energy[my_row / n_atoms], (double)(e + N.blast));
+            if (my_row >= 0) atomicAdd(&energy[my_row / n_atoms], (double)e + (grp == 0 ? (double)N.blast : 0.0));
         }
     }
 
@@ -327,7 +334,7 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
         if (l >= 2) load_w(N.wb[l - 1], Nb, N.dims[l - 1], wbuf[wsel]);   // next operand while the MMAs run
         wait_gemm();
         const float *bl = N.bias[l - 1];
-        for (int c0 = 0; c0 < Nb; c0 += 16) {
+        for (int c0 = grp * 16; c0 < Nb; c0 += 16 * kTcGroups) {
             float d[16], z[16];
             tmem_ld16(tlane + dcol + c0, d);
             tmem_ld16(tlane + N.zoff[l - 1] + c0, z);
@@ -345,7 +352,7 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
             const int n0 = j * 128, nw = min(128, L - n0);
             const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wb[0]);
             const int pieces = (Kb / 8) * nw;
-            for (int t = tid; t < pieces; t += kTM) {
+            for (int t = tid; t < pieces; t += kTcThreads) {
                 const int kc = t / nw, n = t - kc * nw;
                 cp_async16_tc(dst + t * 16, src + ((size_t)kc * L + n0 + n) * 16);
             }
@@ -365,7 +372,7 @@ k_mlp_tc(TcAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_ro
             }
             // tcgen05.ld is warp-collective: rows without an atom take part, only the store is skipped
             float4 *dst = reinterpret_cast<float4 *>(grad + (size_t)(my_row >= 0 ? my_row : 0) * L + n0);
-            for (int c0 = 0; c0 < nw; c0 += 16) {
+            for (int c0 = grp * 16; c0 < nw; c0 += 16 * kTcGroups) {
                 float v[16];
                 tmem_ld16(tlane + n0 + c0, v);
                 if (my_row >= 0) {
@@ -414,17 +421,17 @@ bool mlp_tc_eligible(const MlpNet &n, int L)
     return true;
 }
 
-int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *aev, float *grad_aev,
-                            double *energy_out, cudaStream_t st)
+// Builds the device table of tensor-core operands; called whenever a network is (re)loaded.  Syncs.
+int mlp_tc_upload(aev_ctx *c)
 {
-    const int S = c->dp.S, L = c->dp.L;
+    const int S = c->dp.S;
     TcAll M;
     memset(&M, 0, sizeof(M));
     for (int s = 0; s < S; ++s) {
         const MlpNet &n = c->nets[s];
         TcNetDev &d = M.net[s];
         d.loaded = n.loaded;
-        if (!n.loaded) continue;
+        if (!n.loaded || !n.tc_ok) continue;
         d.nh = n.n_layers - 1;
         for (int l = 0; l <= n.n_layers; ++l) d.dims[l] = n.dims[l];
         int off = 0;
@@ -438,14 +445,24 @@ int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *a
         d.wlast = n.w_f32[d.nh];
         d.blast = n.b_last;
     }
+    if (!c->tc_dev) AEVB_CUDA(cudaMalloc(&c->tc_dev, sizeof(TcAll)));
+    AEVB_CUDA(cudaMemcpy(c->tc_dev, &M, sizeof(TcAll), cudaMemcpyHostToDevice));
+    return AEV_OK;
+}
+
+int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *aev, float *grad_aev,
+                            double *energy_out, cudaStream_t st)
+{
+    const int S = c->dp.S, L = c->dp.L;
+    if (!c->tc_dev) return AEV_ERR_STATE;
     static bool optin = false;
     if (!optin) {
         AEVB_CUDA(cudaFuncSetAttribute(k_mlp_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmem));
         optin = true;
     }
     dim3 grid((n_total + kTM - 1) / kTM, S);
-    k_mlp_tc<<<grid, kTM, kTcSmem, st>>>(M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
-                                          energy_out, c->celu_alpha, c->ws.err);
+    k_mlp_tc<<<grid, kTcThreads, kTcSmem, st>>>(static_cast<const TcAll *>(c->tc_dev), L, n_total, n_atoms, c->sp_rows,
+                                                 c->sp_count, aev, grad_aev, energy_out, c->celu_alpha, c->ws.err);
     return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
 }
 
