@@ -23,45 +23,25 @@ struct MlpDev {
 };
 struct MlpAll { MlpDev net[kMaxS]; };
 
-// Stable partition of the caller's atoms by species: sp_rows[s][0..sp_count[s]) in increasing
-// caller index.  One CTA; each thread owns a contiguous slice.
-__global__ void __launch_bounds__(1024) k_group(int n_total, int S, const int32_t *__restrict__ species,
-                                                int *__restrict__ sp_rows, int *__restrict__ sp_count,
-                                                double *__restrict__ energy, int batch)
+// Partition of the caller's atoms by species: sp_rows[s][0..sp_count[s]).  Slots are handed out
+// with one warp-aggregated atomic per (warp, species); the order inside a species is arbitrary
+// (rows are independent in the GEMMs; the energy sum is an fp64 atomic either way).
+// sp_count must be zero on entry.
+__global__ void __launch_bounds__(256) k_group(int n_total, int S, const int32_t *__restrict__ species,
+                                               int *__restrict__ sp_rows, int *__restrict__ sp_count,
+                                               double *__restrict__ energy, int batch)
 {
-    __shared__ int s_warp[32];
-    __shared__ int s_tot;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    for (int b = tid; b < batch; b += 1024) energy[b] = 0.0;
-    const int per = (n_total + 1023) / 1024;
-    const int beg = min(tid * per, n_total), end = min(beg + per, n_total);
+    const int a = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    if (blockIdx.x == 0)
+        for (int b = threadIdx.x; b < batch; b += blockDim.x) energy[b] = 0.0;
+    const int sp = a < n_total ? species[a] : -1;
     for (int s = 0; s < S; ++s) {
-        int local = 0;
-        for (int a = beg; a < end; ++a) local += (species[a] == s);
-        int incl = local;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            int v = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += v;
-        }
-        if (lane == 31) s_warp[wid] = incl;
-        __syncthreads();
-        if (wid == 0) {
-            int v = s_warp[lane], iv = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int u = __shfl_up_sync(0xffffffffu, iv, o);
-                if (lane >= o) iv += u;
-            }
-            s_warp[lane] = iv - v;
-            if (lane == 31) s_tot = iv;
-        }
-        __syncthreads();
-        int run = s_warp[wid] + incl - local;
-        for (int a = beg; a < end; ++a)
-            if (species[a] == s) sp_rows[(size_t)s * n_total + run++] = a;
-        if (tid == 0) sp_count[s] = s_tot;
-        __syncthreads();
+        const unsigned m = __ballot_sync(0xffffffffu, sp == s);
+        if (m == 0) continue;
+        int base = 0;
+        if (lane == __ffs(m) - 1) base = atomicAdd(&sp_count[s], __popc(m));
+        base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+        if (sp == s) sp_rows[(size_t)s * n_total + base + __popc(m & ((1u << lane) - 1))] = a;
     }
 }
 
@@ -238,7 +218,8 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
         optin = smem;
     }
     prof_begin(c, 5, st);
-    k_group<<<1, 1024, 0, st>>>(n_total, S, species, c->sp_rows, c->sp_count, energy_out, batch);
+    AEVB_CUDA(cudaMemsetAsync(c->sp_count, 0, (size_t)kMaxS * sizeof(int), st));
+    k_group<<<(n_total + 255) / 256, 256, 0, st>>>(n_total, S, species, c->sp_rows, c->sp_count, energy_out, batch);
     // tensor-core path when every loaded network qualifies (ani_mlp_tc.cu); else fp32 CUDA cores
     bool all_tc = true;
     for (int s = 0; s < S; ++s)

@@ -16,6 +16,7 @@
 //   i.e. [K/8][R][8] bf16  =>  descriptor LBO = R*16 (next 8 k), SBO = 128 (next 8 rows).
 #include <cuda_bf16.h>
 #include <math.h>
+#include <stdio.h>
 #include <string.h>
 
 #include <vector>
@@ -26,8 +27,15 @@ using namespace aevb;
 
 namespace {
 
+// -DAEVB_TC_TIMING: CTA (0,0) prints the clock64 offsets of its phase boundaries (debug builds only)
+#ifdef AEVB_TC_TIMING
+#define TC_STAMP(i) do { if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) ts_[i] = clock64() - t0_; } while (0)
+#else
+#define TC_STAMP(i) do { } while (0)
+#endif
+
 constexpr int kTM = 128;              // rows (atoms) per tile = MMA M
-constexpr int kTcGroups = 4;         // warpgroups per CTA: each takes every 4th block of 16 columns in the epilogues
+constexpr int kTcGroups = 8;          // warpgroups per CTA: group g takes the 8-column chunks g, g+8, ... in the epilogues
 constexpr int kTcThreads = kTM * kTcGroups;
 constexpr int kKC = 64;               // K chunk of the first layer (AEV columns per stage)
 constexpr int kActBytes = 81920;      // activation operand: hi | lo, each up to [256/8... K<=160][128][8] bf16
@@ -72,19 +80,17 @@ __device__ __forceinline__ void umma_commit(void *bar)
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                  : "memory");
 }
-__device__ __forceinline__ void tmem_ld16(unsigned taddr, float *v)
+__device__ __forceinline__ void tmem_ld8(unsigned taddr, float *v)      // no wait: pair with tmem_wait()
 {
-    unsigned r[16];
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-        : "r"(taddr)
-        : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    unsigned r[8];
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
 #pragma unroll
-    for (int k = 0; k < 16; ++k) v[k] = __uint_as_float(r[k]);
+    for (int k = 0; k < 8; ++k) v[k] = __uint_as_float(r[k]);
 }
+__device__ __forceinline__ void tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // shared-memory matrix descriptor: no swizzle, K-major, version 1 (sm_100)
 __device__ __forceinline__ unsigned long long smem_desc(unsigned addr, unsigned lbo_bytes, unsigned sbo_bytes)
@@ -103,6 +109,20 @@ __device__ __forceinline__ void cp_async16_tc(void *smem_dst, const void *gsrc)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all_tc() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// 32-byte global accesses (one request per thread: rows are 1.5 KB apart, every lane its own sector)
+__device__ __forceinline__ void ldg256(const float *p, float *v)
+{
+    asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+                 : "l"(p));
+}
+__device__ __forceinline__ void stg256(float *p, const float *v)
+{
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]),
+                 "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7])
+                 : "memory");
+}
 
 // fp32 x8 -> bf16 hi x8 (16 bytes) and bf16 lo x8 (residual)
 __device__ __forceinline__ void split8(const float *v, uint4 &hi, uint4 &lo)
@@ -181,49 +201,59 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
     const unsigned tlane = tmem + ((unsigned)((wid & 3) * 32) << 16);   // this warp's quarter of the 128 lanes
     const int my_row = s_row[row];
     unsigned ph0 = 0, ph1 = 0, ph2 = 0;
+#ifdef AEVB_TC_TIMING
+    __shared__ long long ts_[8];
+    const long long t0_ = clock64();
+#endif
+    TC_STAMP(0);
 
     // ------------------------------------------------------------------ layer 0, K in chunks
     {
         const int K0 = N.dims[0], N1 = N.dims[1];
         const unsigned idesc = instr_desc(N1);
         const int nkc = (K0 + kKC - 1) / kKC;
+        struct F8 { float v[8]; };
+        // this thread's k-chunk (8 AEV columns) of stages kc and kc+1 travel in registers
+        auto load_a = [&](int kc) -> F8 {
+            F8 x;
+            const int col = kc * kKC + grp * 8;
+            if (my_row >= 0 && col < K0) {
+                ldg256(aev + (size_t)my_row * L + col, x.v);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) x.v[k] = 0.f;
+            }
+            return x;
+        };
+        auto load_w0 = [&](int kc) {      // stage kc of W_0: a contiguous block of the [K/8][N][8] operand
+            const int kw = min(kKC, K0 - kc * kKC);
+            const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wf[0]) + (size_t)kc * (kKC / 8) * N1 * 16;
+            unsigned char *dst = wbuf[kc & 1];
+            const int pieces = (kw / 8) * N1;
+            for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
+        };
+        F8 x0 = load_a(0), x1 = load_a(1);
+        load_w0(0);
         for (int kc = 0; kc < nkc; ++kc) {
             const int b = kc & 1;
             const int kw = min(kKC, K0 - kc * kKC);
-            if (kc >= 2) {                 // the MMAs that read this buffer two chunks ago
-                if (b == 0) { mbar_wait(&bar[0], ph0); ph0 ^= 1; } else { mbar_wait(&bar[1], ph1); ph1 ^= 1; }
-            }
             unsigned char *abuf = act + b * 32768;         // hi at +0, lo at +16384
-            unsigned char *wb_ = wbuf[b];
-            {
-                const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wf[0]) + (size_t)kc * (kKC / 8) * N1 * 16;
-                const int pieces = (kw / 8) * N1;
-                for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(wb_ + t * 16, src + (size_t)t * 16);
+            // (the MMAs that read abuf / wbuf[b] two stages ago were waited for in the previous iteration)
+            if (grp < kw / 8) {          // this thread's k-chunk of the stage: columns kc*64 + grp*8 .. +7
+                uint4 hi, lo;
+                split8(x0.v, hi, lo);
+                *reinterpret_cast<uint4 *>(abuf + grp * 2048 + row * 16) = hi;
+                *reinterpret_cast<uint4 *>(abuf + 16384 + grp * 2048 + row * 16) = lo;
             }
-            if (my_row >= 0) {
-                const float4 *src = reinterpret_cast<const float4 *>(aev + (size_t)my_row * L + kc * kKC);
-#pragma unroll 2
-                for (int c = grp; c < kw / 8; c += kTcGroups) {
-                    const float4 x0 = src[2 * c], x1 = src[2 * c + 1];
-                    const float v[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
-                    uint4 hi, lo;
-                    split8(v, hi, lo);
-                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + row * 16) = hi;
-                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + row * 16) = lo;
-                }
-            } else {
-                for (int c = grp; c < kw / 8; c += kTcGroups) {
-                    *reinterpret_cast<uint4 *>(abuf + c * 2048 + row * 16) = make_uint4(0, 0, 0, 0);
-                    *reinterpret_cast<uint4 *>(abuf + 16384 + c * 2048 + row * 16) = make_uint4(0, 0, 0, 0);
-                }
-            }
-            cp_async_wait_all_tc();
+            x0 = x1;
+            x1 = load_a(kc + 2);         // two stages ahead (zeros past the last stage)
+            cp_async_wait_all_tc();      // W_0 stage kc was requested one stage ago
             proxy_fence();
             tc_fence_before();
             __syncthreads();
             if (tid == 0) {
                 tc_fence_after();
-                const unsigned a_hi = smem_u32(abuf), a_lo = a_hi + 16384, b_a = smem_u32(wb_);
+                const unsigned a_hi = smem_u32(abuf), a_lo = a_hi + 16384, b_a = smem_u32(wbuf[b]);
                 for (int ks = 0; ks < kw / 16; ++ks) {
                     const unsigned long long bd = smem_desc(b_a + ks * 2 * N1 * 16, N1 * 16, 128);
                     umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 4096, 2048, 128), bd, idesc, (kc | ks) != 0);
@@ -231,17 +261,23 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
                 }
                 umma_commit(&bar[b]);
             }
+            if (kc + 1 < nkc) {
+                // the other buffer pair is free once the MMAs of stage kc-1 are done; then prefetch W_0 stage kc+1
+                if (kc >= 1) {
+                    if (b == 1) { mbar_wait(&bar[0], ph0); ph0 ^= 1; } else { mbar_wait(&bar[1], ph1); ph1 ^= 1; }
+                }
+                load_w0(kc + 1);
+            }
         }
-        // drain: every outstanding commit (at most one per buffer)
+        // drain the commits not waited for above: stage nkc-2 (if any), then stage nkc-1
         if (nkc >= 2) {
-            mbar_wait(&bar[0], ph0); ph0 ^= 1;
-            mbar_wait(&bar[1], ph1); ph1 ^= 1;
-        } else {
-            mbar_wait(&bar[0], ph0); ph0 ^= 1;
+            if (((nkc - 2) & 1) == 0) { mbar_wait(&bar[0], ph0); ph0 ^= 1; } else { mbar_wait(&bar[1], ph1); ph1 ^= 1; }
         }
+        if (((nkc - 1) & 1) == 0) { mbar_wait(&bar[0], ph0); ph0 ^= 1; } else { mbar_wait(&bar[1], ph1); ph1 ^= 1; }
         tc_fence_after();
     }
 
+    TC_STAMP(1);
     // whole-layer weight operand -> shared memory (contiguous [K/8][N][8] block)
     auto load_w = [&](const __nv_bfloat16 *w, int K, int Nn, unsigned char *dst) {
         const unsigned char *src = reinterpret_cast<const unsigned char *>(w);
@@ -267,15 +303,12 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
         ph2 ^= 1;
         tc_fence_after();
     };
-    // 16 fp32 values of this thread's row -> operand columns c0..c0+15 (hi and lo)
-    auto put16 = [&](const float *v, int c0) {
+    // 8 fp32 values of this thread's row -> operand k-chunk c (columns 8c..8c+7), hi and lo
+    auto put8 = [&](const float *v, int c) {
         uint4 hi, lo;
         split8(v, hi, lo);
-        *reinterpret_cast<uint4 *>(act + (c0 >> 3) * 2048 + row * 16) = hi;
-        *reinterpret_cast<uint4 *>(act + kActHalf + (c0 >> 3) * 2048 + row * 16) = lo;
-        split8(v + 8, hi, lo);
-        *reinterpret_cast<uint4 *>(act + ((c0 >> 3) + 1) * 2048 + row * 16) = hi;
-        *reinterpret_cast<uint4 *>(act + kActHalf + ((c0 >> 3) + 1) * 2048 + row * 16) = lo;
+        *reinterpret_cast<uint4 *>(act + c * 2048 + row * 16) = hi;
+        *reinterpret_cast<uint4 *>(act + kActHalf + c * 2048 + row * 16) = lo;
     };
     auto sync_for_mma = [&]() {      // generic-proxy writes + cp.async data visible to the tensor core
         cp_async_wait_all_tc();
@@ -283,50 +316,77 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
         tc_fence_before();
         __syncthreads();
     };
+    constexpr int kMaxC = 3;         // 8-column chunks per thread in a hidden-layer epilogue (width <= 160... 192)
 
     // ------------------------------------------------------------------ forward, layers 1 .. nh-1
     int wsel = 0;
     for (int l = 1; l <= nh; ++l) {
         // z_l (output of layer l-1) is complete in TMEM at zoff[l-1]
-        const int Nl = N.dims[l];
+        const int Nl = N.dims[l], ncl = Nl >> 3;
         const float *bl = N.bias[l - 1];
-        if (l < nh) {
-            load_w(N.wf[l], Nl, N.dims[l + 1], wbuf[wsel]);               // overlaps the epilogue below
-            for (int c0 = grp * 16; c0 < Nl; c0 += 16 * kTcGroups) {
-                float v[16];
-                tmem_ld16(tlane + N.zoff[l - 1] + c0, v);
+        if (l < nh) load_w(N.wf[l], Nl, N.dims[l + 1], wbuf[wsel]);               // overlaps the epilogue below
+        else if (nh >= 2) load_w(N.wb[nh - 1], Nl, N.dims[nh - 1], wbuf[wsel]);
+        float v[kMaxC][8];
 #pragma unroll
-                for (int k = 0; k < 16; ++k) v[k] = celu_tc(v[k] + __ldg(bl + c0 + k), alpha, inv_alpha);
-                put16(v, c0);
+        for (int i = 0; i < kMaxC; ++i) {
+            const int c = grp + i * kTcGroups;
+            if (c < ncl) tmem_ld8(tlane + N.zoff[l - 1] + c * 8, v[i]);
+        }
+        tmem_wait();
+        float e = 0.f;
+#pragma unroll
+        for (int i = 0; i < kMaxC; ++i) {
+            const int c = grp + i * kTcGroups;
+            if (c < ncl) {
+                const float4 b0 = __ldg(reinterpret_cast<const float4 *>(bl + c * 8));
+                const float4 b1 = __ldg(reinterpret_cast<const float4 *>(bl + c * 8) + 1);
+                const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+                if (l < nh) {
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) v[i][k] = celu_tc(v[i][k] + bb[k], alpha, inv_alpha);
+                } else {
+                    // last hidden layer: energy (the N = 1 layer, CUDA cores) and d_nh = w_last * CELU'(z)
+                    const float4 w0 = __ldg(reinterpret_cast<const float4 *>(N.wlast + c * 8));
+                    const float4 w1 = __ldg(reinterpret_cast<const float4 *>(N.wlast + c * 8) + 1);
+                    const float ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const float z = v[i][k] + bb[k];
+                        e = fmaf(celu_tc(z, alpha, inv_alpha), ww[k], e);
+                        v[i][k] = ww[k] * dcelu_tc(z, inv_alpha);
+                    }
+                }
+                put8(v[i], c);
             }
+        }
+        if (l < nh) {
             sync_for_mma();
             gemm(Nl, N.dims[l + 1], wbuf[wsel], N.dims[l + 1] * 16, N.zoff[l]);
             wsel ^= 1;
             wait_gemm();
         } else {
-            // last hidden layer: energy (N = 1 layer on the CUDA cores) and d_nh = w_last * CELU'(z)
-            if (nh >= 2) load_w(N.wb[nh - 1], Nl, N.dims[nh - 1], wbuf[wsel]);
-            float e = 0.f;
-            for (int c0 = grp * 16; c0 < Nl; c0 += 16 * kTcGroups) {
-                float v[16];
-                tmem_ld16(tlane + N.zoff[l - 1] + c0, v);
+            // energy: one fp64 atomic per warp when its rows belong to one system (the usual case)
+            double ed = my_row >= 0 ? (double)e + (grp == 0 ? (double)N.blast : 0.0) : 0.0;
+            const int bsys = my_row >= 0 ? my_row / n_atoms : -1;
+            const unsigned have = __ballot_sync(0xffffffffu, my_row >= 0);
+            if (have) {
+                const int b0 = __shfl_sync(0xffffffffu, bsys, __ffs(have) - 1);
+                if (__all_sync(0xffffffffu, bsys == b0 || bsys < 0)) {
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                    const float z = v[k] + __ldg(bl + c0 + k);
-                    const float w = __ldg(N.wlast + c0 + k);
-                    e = fmaf(celu_tc(z, alpha, inv_alpha), w, e);
-                    v[k] = w * dcelu_tc(z, inv_alpha);
+                    for (int o = 16; o >= 1; o >>= 1) ed += __shfl_xor_sync(0xffffffffu, ed, o);
+                    if ((tid & 31) == 0) atomicAdd(&energy[b0], ed);
+                } else if (my_row >= 0) {
+                    atomicAdd(&energy[bsys], ed);
                 }
-                put16(v, c0);
             }
-            if (my_row >= 0) atomicAdd(&energy[my_row / n_atoms], (double)e + (grp == 0 ? (double)N.blast : 0.0));
         }
     }
 
+    TC_STAMP(2);
     // ------------------------------------------------------------------ backward, layers nh-1 .. 1
     for (int l = nh - 1; l >= 1; --l) {
-        // act holds d_(l+1) [128 x dims[l+1]]; wbuf[wsel] holds (or is receiving) W_l^T operand
-        const int Kb = N.dims[l + 1], Nb = N.dims[l];
+        // act holds d_(l+1) [128 x dims[l+1]]; wbuf[wsel] holds (or is receiving) the W_l^T operand
+        const int Kb = N.dims[l + 1], Nb = N.dims[l], ncl = Nb >> 3;
         const unsigned dcol = N.zoff[l];                   // z_(l+1) is dead: reuse its columns
         sync_for_mma();
         gemm(Kb, Nb, wbuf[wsel], Nb * 16, dcol);
@@ -334,16 +394,25 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
         if (l >= 2) load_w(N.wb[l - 1], Nb, N.dims[l - 1], wbuf[wsel]);   // next operand while the MMAs run
         wait_gemm();
         const float *bl = N.bias[l - 1];
-        for (int c0 = grp * 16; c0 < Nb; c0 += 16 * kTcGroups) {
-            float d[16], z[16];
-            tmem_ld16(tlane + dcol + c0, d);
-            tmem_ld16(tlane + N.zoff[l - 1] + c0, z);
 #pragma unroll
-            for (int k = 0; k < 16; ++k) d[k] *= dcelu_tc(z[k] + __ldg(bl + c0 + k), inv_alpha);
-            put16(d, c0);
+        for (int i = 0; i < kMaxC; ++i) {
+            const int c = grp + i * kTcGroups;
+            if (c < ncl) {
+                float d[8], z[8];
+                tmem_ld8(tlane + dcol + c * 8, d);
+                tmem_ld8(tlane + N.zoff[l - 1] + c * 8, z);
+                const float4 b0 = __ldg(reinterpret_cast<const float4 *>(bl + c * 8));
+                const float4 b1 = __ldg(reinterpret_cast<const float4 *>(bl + c * 8) + 1);
+                const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+                tmem_wait();
+#pragma unroll
+                for (int k = 0; k < 8; ++k) d[k] *= dcelu_tc(z[k] + bb[k], inv_alpha);
+                put8(d, c);
+            }
         }
     }
 
+    TC_STAMP(3);
     // ------------------------------------------------------------------ d_0 = d_1 W_0^T, N = L in chunks of 128
     {
         const int Kb = N.dims[1];
@@ -371,18 +440,27 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
                 wsel ^= 1;
             }
             // tcgen05.ld is warp-collective: rows without an atom take part, only the store is skipped
-            float4 *dst = reinterpret_cast<float4 *>(grad + (size_t)(my_row >= 0 ? my_row : 0) * L + n0);
-            for (int c0 = grp * 16; c0 < nw; c0 += 16 * kTcGroups) {
-                float v[16];
-                tmem_ld16(tlane + n0 + c0, v);
-                if (my_row >= 0) {
+            float *dst = grad + (size_t)(my_row >= 0 ? my_row : 0) * L + n0;
+            float v[2][8];
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) dst[(c0 >> 2) + k] = make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
-                }
+            for (int i = 0; i < 2; ++i) {
+                const int c = grp + i * kTcGroups;
+                if (c * 8 < nw) tmem_ld8(tlane + n0 + c * 8, v[i]);
+            }
+            tmem_wait();
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int c = grp + i * kTcGroups;
+                if (c * 8 < nw && my_row >= 0) stg256(dst + c * 8, v[i]);
             }
         }
     }
 
+    TC_STAMP(4);
+#ifdef AEVB_TC_TIMING
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0)
+        printf("TC %lld %lld %lld %lld %lld\n", ts_[0], ts_[1], ts_[2], ts_[3], ts_[4]);
+#endif
     // ------------------------------------------------------------------ teardown
     tc_fence_before();
     __syncthreads();
