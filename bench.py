@@ -290,8 +290,10 @@ def run_ours(args):
     prof = ctx.aev_get_profile()
     ctx.aev_set_profiling(False)
     kern_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in prof.items()}
-    dom = "backward" if kern_ms["backward"] >= kern_ms["forward"] else "forward"
-    dom_flop = flop_bwd if dom == "backward" else flop_fwd
+    flop_nbr = FLOP_CAND * wc["candidates"]
+    kflop = {"nbr": flop_nbr, "aev": flop_fwd - flop_nbr, "backward": flop_bwd}
+    dom = max(kflop, key=lambda k: kern_ms[k])
+    dom_flop = kflop[dom]
     achieved = dom_flop / (kern_ms[dom] * 1e-3) / 1e12
     try:
         probe = pkg.probe_fp32_tflops(local)
