@@ -130,6 +130,11 @@ def _work_counts(counts: np.ndarray, pos: np.ndarray, box, rcr: float):
     return {"radial_pairs_directed": p_r, "angular_pairs_directed": p_a, "triplets": trip, "candidates": cand}
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on C4, from the one `ncu --set full` capture
+# summarised in profiles/r1_final_ncu_full.md (bench.py never runs under a profiler itself)
+NCU_TRAFFIC_BYTES = {"backward": 61.2e6 + 0.51e6, "aev": 24.9e6 + 0.24e6, "nbr": 0.53e6 + 0.01e6}
+
+
 def _flops(wc):
     fwd = FLOP_PAIR_FWD * wc["radial_pairs_directed"] + FLOP_TRIPLET_FWD * wc["triplets"] \
         + 0.5 * FLOP_APAIR * wc["angular_pairs_directed"] + FLOP_CAND * wc["candidates"]
@@ -301,7 +306,7 @@ def run_ours(args):
         probe = None
     roofline = {
         "bound": "alu", "kernel": "k_" + dom, "achieved": achieved, "peak": ALU_PEAK_TFLOPS,
-        "unit": "TFLOP/s", "frac": achieved / ALU_PEAK_TFLOPS, "traffic": None,
+        "unit": "TFLOP/s", "frac": achieved / ALU_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(dom),
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 7)",
         "fma_probe_tflops": probe,
         "algorithmic_flop_per_launch": dom_flop,
