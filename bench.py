@@ -202,6 +202,20 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def aggregate_over_ranks(total_ms, units_per_rank, steps, dist, device=None):
+    """Whole-job throughput of N independent replicas (replicas only, no
+    data-path collective): the timed region of the job is the MAX over ranks, the units are the
+    SUM over ranks.  `dist` is torch.distributed (initialised) or None for one process."""
+    import torch
+    world = 1
+    if dist is not None:
+        world = dist.get_world_size()
+        t = torch.tensor([float(total_ms)], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    return total_ms, world * units_per_rank * steps / (total_ms * 1e-3)
+
+
 def _time_steps(fn, steps, flush, torch):
     """Per-step CUDA-event timing on the current stream; L2 flushed before every step."""
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
@@ -269,12 +283,7 @@ def run_ours(args):
     launches = ctx.launch_count() - l0
     barrier()
     clocks = sampler.stop()
-    total_ms = float(t_ms.sum())
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    value = world * n_atoms * args.steps / (total_ms * 1e-3)
+    total_ms, value = aggregate_over_ranks(float(t_ms.sum()), n_atoms, args.steps, dist, dev)
     ctx.check_status()
 
     if rank != 0:

@@ -233,3 +233,63 @@ def test_c5_energy_and_forces(pkg):
     assert abs(e2[0] - e[0]) <= 1e-9 * max(1.0, abs(e[0]))
     np.testing.assert_allclose(f2, f, rtol=0, atol=1e-5 * np.abs(f).max())   # RED order
     ctx.close()
+
+
+def test_mlp_fp32_path_for_weights_that_are_not_bf16(pkg):
+    """Weights that are not bf16-representable must not be rounded: the library runs the fp32
+    CUDA-core kernel for them and stays within the fp32 force tolerance."""
+    w = make_workload("C5")
+    nets = make_c5_weights()
+    rng = np.random.default_rng(7)
+    nets = {s: ([(x * (1.0 + 2.0 ** -11 * rng.standard_normal(x.shape))).astype(np.float32) for x in ws], bs)
+            for s, (ws, bs) in nets.items()}
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    pos, sp, _ = _dev(w)
+    e, f = ctx.ani_energy_forces(pos, sp, w.box)
+    ctx.check_status()
+    e, f = e.cpu().numpy(), f.cpu().numpy().astype(np.float64)
+    we, wf, _ = oracle.energy_forces(w.params, w.pos, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
+    assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    assert _rel_rms(f, wf) <= FORCE_TOL
+    ctx.close()
+
+
+def test_mlp_tensor_core_path_other_depths(pkg):
+    """One and two hidden layers, widths that are not powers of two (tcgen05 N = 160, 96, 48)."""
+    w = make_workload("C5")
+    nets = make_c5_weights(seed=3, arch={0: [384, 96, 48, 1], 3: [384, 160, 1]})
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    pos, sp, _ = _dev(w)
+    e, f = ctx.ani_energy_forces(pos, sp, w.box)
+    ctx.check_status()
+    e, f = e.cpu().numpy(), f.cpu().numpy().astype(np.float64)
+    we, wf, _ = oracle.energy_forces(w.params, w.pos, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
+    assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    assert _rel_rms(f, wf) <= C5_FORCE_TOL
+    ctx.close()
+
+
+def test_large_gas_phase_cluster_uses_the_unstaged_scan(pkg):
+    """1,200 atoms without a box: one cell whose 1,200 candidates exceed the shared-memory stage,
+    so k_nbr takes its global-memory ballot path; pair sets stay bit-exact."""
+    from gen import make_water_box
+    wb = make_water_box(400, 24.0, 910, "cluster")
+    pos, sp, g = _dev(wb)
+    ctx = pkg.Context(wb.params, max_atoms=wb.n_atoms)
+    aev = ctx.aev_forward(pos, sp, None)
+    forces = ctx.aev_backward(g)
+    ctx.check_status()
+    for which, rc in ((0, wb.params.rcr), (1, wb.params.rca)):
+        got = ctx.aev_export_pairs(which, cap=wb.n_atoms * 64)
+        want = oracle.pairs(wb.pos[0], wb.species[0], None, float(rc), "brute").astype(np.int32)
+        np.testing.assert_array_equal(got, want)
+    want_aev = oracle.aev_forward(wb.params, wb.pos, wb.species, None, use_cells=False)
+    want_f = oracle.aev_backward(wb.params, wb.pos, wb.species, None, wb.grad_aev, use_cells=False)
+    a = aev.cpu().numpy().astype(np.float64)
+    assert np.abs(a - want_aev).max() / np.abs(want_aev).max() <= AEV_TOL
+    assert _rel_rms(forces.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    ctx.close()
