@@ -90,7 +90,9 @@ struct aev_ctx {
     cudaStream_t last_stream;
     size_t cap_total;            // atoms the workspace is sized for
     size_t nbins_cap, members_cap;
-    int fwd_smem_optin;          // bytes of dynamic smem the forward kernel was opted into
+    int fwd_smem_optin;          // bytes of dynamic smem the forward kernels were opted into (per device => per ctx)
+    size_t bwd_smem_optin, mlp_smem_optin;
+    int tc_smem_optin;
     // MLP
     aevb::MlpNet nets[aevb::kMaxS];
     float celu_alpha;

@@ -212,10 +212,9 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
     }
     constexpr int TM = 8;
     const size_t smem = (size_t)TM * sum_hidden * sizeof(float);
-    static size_t optin = 0;
-    if (smem > optin) {
+    if (smem > c->mlp_smem_optin) {
         AEVB_CUDA(cudaFuncSetAttribute(k_mlp_f32<TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        optin = smem;
+        c->mlp_smem_optin = smem;
     }
     prof_begin(c, 5, st);
     AEVB_CUDA(cudaMemsetAsync(c->sp_count, 0, (size_t)kMaxS * sizeof(int), st));

@@ -533,10 +533,9 @@ int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *a
 {
     const int S = c->dp.S, L = c->dp.L;
     if (!c->tc_dev) return AEV_ERR_STATE;
-    static bool optin = false;
-    if (!optin) {
+    if (!c->tc_smem_optin) {
         AEVB_CUDA(cudaFuncSetAttribute(k_mlp_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmem));
-        optin = true;
+        c->tc_smem_optin = 1;
     }
     dim3 grid((n_total + kTM - 1) / kTM, S);
     k_mlp_tc<<<grid, kTcThreads, kTcSmem, st>>>(static_cast<const TcAll *>(c->tc_dev), L, n_total, n_atoms, c->sp_rows,
