@@ -338,16 +338,20 @@ def run_ours(args):
     # ---- end to end through the host-buffer entry point (pinned staging inside the library)
     e2e_steps = max(3, min(args.steps, 20))
     ctx.aev_forward_backward_host(w.pos, w.species, w.box, w.grad_aev)
-    aev_h = np.empty((w.batch, w.n_atoms, ctx.length), dtype=np.float32)
-    f_h = np.empty((w.batch, w.n_atoms, 3), dtype=np.float32)
+    # the caller's buffers are page-locked host memory (the library copies from / to them directly)
+    pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
+    pos_h, sp_h, g_h = pin(w.pos), pin(w.species), pin(w.grad_aev)
+    aev_h = torch.empty((w.batch, w.n_atoms, ctx.length), dtype=torch.float32).pin_memory().numpy()
+    f_h = torch.empty((w.batch, w.n_atoms, 3), dtype=torch.float32).pin_memory().numpy()
+    ctx.aev_forward_backward_host(pos_h, sp_h, w.box, g_h, aev_out=aev_h, forces_out=f_h)
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        ctx.aev_forward_backward_host(w.pos, w.species, w.box, w.grad_aev, aev_out=aev_h, forces_out=f_h)
+        ctx.aev_forward_backward_host(pos_h, sp_h, w.box, g_h, aev_out=aev_h, forces_out=f_h)
     dt = time.perf_counter() - t0
     e2e = {"value": n_atoms * e2e_steps / dt, "unit": UNIT, "steps": e2e_steps,
            "h2d_bytes_per_step": int(w.pos.nbytes + w.species.nbytes + w.grad_aev.nbytes),
            "d2h_bytes_per_step": int(aev_h.nbytes + f_h.nbytes),
-           "call": "aev_forward_backward_host (host pointers; pinned staging + H2D + kernels + D2H, synchronous)"}
+           "call": "aev_forward_backward_host (pinned host pointers; H2D of grad || forward kernels || D2H of the AEV, then backward + D2H of the forces; synchronous)"}
 
     # ---- the other configurations (context rows, not the headline)
     other = {}

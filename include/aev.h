@@ -151,6 +151,10 @@ int ani_energy_forces(aev_ctx *c, const float *pos, const int32_t *species, cons
  * pointer is a HOST pointer; the library stages through pinned buffers and device
  * workspace it owns, runs the same kernels, and copies the results back.  They sync.
  * Any of aev_out / grad_aev+forces_out may be NULL to skip that half.
+ * Page-locked host buffers (cudaHostAlloc, cudaHostRegister, torch pin_memory) are copied from /
+ * to directly; pageable ones are staged through the context's pinned buffer.  The copy of
+ * grad_aev, the forward kernels and the read-back of aev_out run on three streams of the
+ * context, so the two PCIe directions overlap each other and the kernels.
  */
 int aev_forward_backward_host(aev_ctx *c, const float *pos, const int32_t *species,
                               const float *box, int32_t n_atoms, int32_t batch,

@@ -109,6 +109,8 @@ struct aev_ctx {
     void *prof;                  // std::vector<ProfRec>* (aev_kernels.cu)
     void *h_pin; size_t h_pin_bytes;
     void *d_stage; size_t d_stage_bytes;
+    cudaStream_t s_main, s_h2d, s_d2h;      // streams of the host entry points (kernels, big H2D, big D2H)
+    cudaEvent_t ev_fwd, ev_grad;
 };
 
 namespace aevb {
