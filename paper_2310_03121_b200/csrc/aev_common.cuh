@@ -15,7 +15,7 @@ constexpr int kNA = 4;         // angular radial shifts
 constexpr int kNZ = 8;         // angular angle shifts
 constexpr int kBlk = kNA * kNZ;  // 32 entries per species-pair block
 constexpr int kMaxS = 8;
-constexpr int kSpeciesShift = 26;  // neighbour entry .w = j_sorted | species << 26
+constexpr int kSpeciesShift = 26;  // neighbour entry .w = caller index of j | species << 26
 constexpr int kIdxMask = (1 << kSpeciesShift) - 1;
 constexpr int kMaxMlpLayers = 4;
 
@@ -48,15 +48,11 @@ struct Geom {
 // Device workspace owned by the context.
 struct Workspace {
     float4 *wpos;        // [n_total] wrapped position + species bits (caller order)
-    int *bin_of;         // [n_total] bin id of each atom or -1
-    int *bin_cnt;        // [nbins_cap] member counts (zero between calls)
+    int *bin_cnt;        // [2][nbins_cap] member counts, double-buffered by call parity
     int *members;        // [nbins_cap*bin_cap] caller index of bin members
-    int *bin_start;      // [nbins_cap+1] exclusive scan of bin_cnt
-    float4 *spos;        // [n_total] sorted positions, .w = caller index bits
-    int *perm;           // [n_total] sorted -> caller flat index
     float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, caller index j | s<<26), angular first
     int2 *ncount;        // [n_total] (nA, nB)
-    int4 *hdr;           // [n_total] per sorted atom: (nA, nB, caller index, species)
+    int4 *hdr;           // [n_total] per atom (caller order): (nA, nB, caller index, species)
     int *noff;           // [n_total][kMaxS+1] per-species list offsets: offA | offB << 16
     int *err;            // device error flags (bitmask)
     unsigned long long *pair_count;  // export counter
@@ -90,6 +86,7 @@ struct aev_ctx {
     cudaStream_t last_stream;
     size_t cap_total;            // atoms the workspace is sized for
     size_t nbins_cap, members_cap;
+    int bin_parity;              // which half of ws.bin_cnt the next call counts into
     int fwd_smem_optin;          // bytes of dynamic smem the forward kernels were opted into (per device => per ctx)
     size_t bwd_smem_optin, mlp_smem_optin;
     int tc_smem_optin;
