@@ -370,6 +370,25 @@ def run_ours(args):
         tt = _time_steps(st2, min(args.steps, 50), flush, torch)
         other[name] = {"ms_per_eval": float(tt.mean()), "atoms_per_s": ww.batch * ww.n_atoms / (tt.mean() * 1e-3),
                        "evaluations_per_s": ww.batch / (tt.mean() * 1e-3)}
+        # the same evaluation captured once in a CUDA graph and replayed (the MD-loop calling pattern)
+        try:
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                st2()
+            torch.cuda.current_stream().wait_stream(side)
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                st2()
+            for _ in range(3):
+                graph.replay()
+            tg = _time_steps(graph.replay, min(args.steps, 50), flush, torch)
+            c2.check_status()
+            other[name]["graph_ms_per_eval"] = float(tg.mean())
+            other[name]["graph_evaluations_per_s"] = ww.batch / (tg.mean() * 1e-3)
+            del graph
+        except Exception as exc:      # reported, never fatal for the headline
+            other[name]["graph_error"] = repr(exc)[:200]
         c2.close()
     w5 = make_workload("C5")
     c5 = pkg.Context(w5.params, max_atoms=w5.n_atoms, device=local)

@@ -48,13 +48,14 @@ struct Geom {
 // Device workspace owned by the context.
 struct Workspace {
     float4 *wpos;        // [n_total] wrapped position + species bits (caller order)
-    int *bin_cnt;        // [2][nbins_cap] member counts, double-buffered by call parity
+    int *bin_cnt;        // [nbins_cap] member counts (zero between calls: cleared by k_nbr)
     int *members;        // [nbins_cap*bin_cap] caller index of bin members
     float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, caller index j | s<<26), angular first
     int2 *ncount;        // [n_total] (nA, nB)
     int4 *hdr;           // [n_total] per atom (caller order): (nA, nB, caller index, species)
     int *noff;           // [n_total][kMaxS+1] per-species list offsets: offA | offB << 16
     int *err;            // device error flags (bitmask)
+    unsigned *nbr_done;  // k_nbr CTAs that have read their bin counters (reset by the last one)
     unsigned long long *pair_count;  // export counter
 };
 
@@ -86,7 +87,6 @@ struct aev_ctx {
     cudaStream_t last_stream;
     size_t cap_total;            // atoms the workspace is sized for
     size_t nbins_cap, members_cap;
-    int bin_parity;              // which half of ws.bin_cnt the next call counts into
     int fwd_smem_optin;          // bytes of dynamic smem the forward kernels were opted into (per device => per ctx)
     size_t bwd_smem_optin, mlp_smem_optin;
     int tc_smem_optin;
