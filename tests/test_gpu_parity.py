@@ -293,3 +293,30 @@ def test_large_gas_phase_cluster_uses_the_unstaged_scan(pkg):
     assert np.abs(a - want_aev).max() / np.abs(want_aev).max() <= AEV_TOL
     assert _rel_rms(forces.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
     ctx.close()
+
+
+@pytest.mark.gpu
+def test_seven_species_ani2x_shape(pkg):
+    """S = 7 (ANI-2x-shaped AEV, L = 7*16 + 28*32 = 1008): the neighbour kernel's
+    64-bit packed species fields and 28 species-pair blocks, gas phase and periodic."""
+    p7 = ani1x_style_params(num_species=7)
+    assert p7.aev_length == 1008
+    rng = np.random.default_rng(77)
+    for name in ("C1", "C3"):
+        w = make_workload(name)
+        sp = rng.integers(0, 7, size=w.species.shape).astype(np.int32)
+        g = rng.standard_normal((w.batch, w.n_atoms, 1008)).astype(np.float32)
+        ctx = pkg.Context(p7, max_atoms=w.n_atoms, max_batch=w.batch)
+        pos_d, sp_d = torch.from_numpy(w.pos).cuda(), torch.from_numpy(sp).cuda()
+        aev = ctx.aev_forward(pos_d, sp_d, w.box)
+        f = ctx.aev_backward(torch.from_numpy(g).cuda())
+        ctx.check_status()
+        for which, rc in ((0, p7.rcr), (1, p7.rca)):
+            got = ctx.aev_export_pairs(which, cap=w.n_atoms * 64)
+            want = oracle.pairs(w.pos[0], sp[0], w.box, float(rc), "brute")
+            np.testing.assert_array_equal(got, want.astype(np.int32))
+        want_a = oracle.aev_forward(p7, w.pos, sp, w.box, use_cells=w.box is not None)
+        want_f = oracle.aev_backward(p7, w.pos, sp, w.box, g, use_cells=w.box is not None)
+        assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+        assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+        ctx.close()
