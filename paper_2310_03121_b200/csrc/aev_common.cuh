@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "../../include/aev.h"
 
@@ -119,6 +120,27 @@ namespace aevb {
     } while (0)
 
 enum { kErrBitCapacity = 1, kErrBitState = 2 };
+
+// Programmatic dependent launch: a kernel launched with launch_pdl() may become resident while its
+// predecessor in the stream is still draining; it must pass pdl_wait() before it touches anything the
+// predecessor (or, transitively, an earlier kernel) wrote.  pdl_trigger() lets the successor start early.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
+// species partition for the MLP (ani_mlp.cu): memset of the counters + k_group
+int mlp_group(aev_ctx *c, const int32_t *species, int n_total, int batch, double *energy_out, cudaStream_t st);
 
 // MLP entry points implemented in ani_mlp.cu
 int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_atoms, int batch,

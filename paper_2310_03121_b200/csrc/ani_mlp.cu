@@ -63,6 +63,8 @@ k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_
           double *__restrict__ energy, float alpha, int *__restrict__ err)
 {
     extern __shared__ __align__(16) float sm[];
+    pdl_trigger();
+    pdl_wait();               // the AEV rows (k_aev) are complete
     const int s = blockIdx.y;
     const int rows = sp_count[s];
     const int r0 = blockIdx.x * TM;
@@ -191,6 +193,14 @@ void mlp_free(aev_ctx *c)
     }
 }
 
+int mlp_group(aev_ctx *c, const int32_t *species, int n_total, int batch, double *energy_out, cudaStream_t st)
+{
+    AEVB_CUDA(cudaMemsetAsync(c->sp_count, 0, (size_t)kMaxS * sizeof(int), st));
+    k_group<<<(n_total + 255) / 256, 256, 0, st>>>(n_total, c->dp.S, species, c->sp_rows, c->sp_count, energy_out, batch);
+    c->launches += 1;
+    return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
+}
+
 int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_atoms, int batch,
                          const float *aev, float *grad_aev, double *energy_out, cudaStream_t st)
 {
@@ -217,8 +227,6 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
         c->mlp_smem_optin = smem;
     }
     prof_begin(c, 5, st);
-    AEVB_CUDA(cudaMemsetAsync(c->sp_count, 0, (size_t)kMaxS * sizeof(int), st));
-    k_group<<<(n_total + 255) / 256, 256, 0, st>>>(n_total, S, species, c->sp_rows, c->sp_count, energy_out, batch);
     // tensor-core path when every loaded network qualifies (ani_mlp_tc.cu); else fp32 CUDA cores
     bool all_tc = true;
     for (int s = 0; s < S; ++s)
@@ -226,14 +234,14 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
     if (all_tc && !getenv("AEVB_MLP_FP32")) {
         const int rc = mlp_tc_forward_backward(c, n_total, n_atoms, aev, grad_aev, energy_out, st);
         prof_end(c, st);
-        c->launches += 2;
+        c->launches += 1;
         return rc;
     }
     dim3 grid((n_total + TM - 1) / TM, S);
-    k_mlp_f32<TM><<<grid, 256, smem, st>>>(M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
-                                            energy_out, c->celu_alpha, c->ws.err);
+    launch_pdl(k_mlp_f32<TM>, grid, dim3(256), smem, st, M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
+               energy_out, c->celu_alpha, c->ws.err);
     prof_end(c, st);
-    c->launches += 2;
+    c->launches += 1;
     if (cudaGetLastError() != cudaSuccess) return AEV_ERR_CUDA;
     return AEV_OK;
 }

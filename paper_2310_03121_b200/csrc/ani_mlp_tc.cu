@@ -166,6 +166,8 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
 {
     extern __shared__ __align__(1024) unsigned char sm[];
     __shared__ int s_row[kTM];
+    pdl_trigger();
+    pdl_wait();               // the AEV rows (k_aev) are complete
     const int s = blockIdx.y;
     const int rows = sp_count[s];
     const int r0 = blockIdx.x * kTM;
@@ -538,8 +540,9 @@ int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *a
         c->tc_smem_optin = 1;
     }
     dim3 grid((n_total + kTM - 1) / kTM, S);
-    k_mlp_tc<<<grid, kTcThreads, kTcSmem, st>>>(static_cast<const TcAll *>(c->tc_dev), L, n_total, n_atoms, c->sp_rows,
-                                                 c->sp_count, aev, grad_aev, energy_out, c->celu_alpha, c->ws.err);
+    launch_pdl(k_mlp_tc, grid, dim3(kTcThreads), (size_t)kTcSmem, st, static_cast<const TcAll *>(c->tc_dev), L, n_total,
+               n_atoms, (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->celu_alpha,
+               c->ws.err);
     return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
 }
 
