@@ -320,3 +320,35 @@ def test_seven_species_ani2x_shape(pkg):
         assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
         assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
         ctx.close()
+
+
+@pytest.mark.gpu
+def test_large_box_is_periodic_replication(pkg):
+    """288,000 atoms: C3's box replicated 4x4x4 (L = 142 A, 27^3 cells x 4 species = 78,732 bins). Every atom
+    of a replica has the environment of its original, so the first replica's rows must equal the 4,500-atom
+    oracle result (coordinates shifted by up to 3 box lengths perturb fp32 positions by ~1e-5 A)."""
+    w = make_workload("C3")
+    L0 = np.asarray(w.box, dtype=np.float64)
+    reps = 4
+    shifts = np.array([[i, j, k] for i in range(reps) for j in range(reps) for k in range(reps)], dtype=np.float64)
+    pos = (w.pos[0].astype(np.float64)[None] + (shifts * L0)[:, None, :]).reshape(1, -1, 3).astype(np.float32)
+    sp = np.tile(w.species[0], reps ** 3)[None].astype(np.int32)
+    box = (L0 * reps).astype(np.float32)
+    n = pos.shape[1]
+    ctx = pkg.Context(w.params, max_atoms=n)
+    aev = ctx.aev_forward(torch.from_numpy(pos).cuda(), torch.from_numpy(sp).cuda(), box)
+    g = torch.zeros_like(aev)
+    g[0, :w.n_atoms] = torch.from_numpy(w.grad_aev[0]).cuda()
+    f = ctx.aev_backward(g)
+    ctx.check_status()
+    counts = ctx.aev_export_counts(1, n).cpu().numpy().reshape(n, 2)
+    a0 = aev[0, :w.n_atoms].cpu().numpy().astype(np.float64)
+    want = oracle.aev_forward(w.params, w.pos, w.species, w.box, use_cells=True)[0]
+    assert np.abs(a0 - want).max() <= 2e-3 * np.abs(want).max()
+    # all 64 replicas have identical neighbour counts
+    c = counts.reshape(reps ** 3, w.n_atoms, 2)
+    assert np.all(c == c[0][None])
+    # forces: upstream gradient only on the first replica's rows; total force is zero
+    ff = f[0].cpu().numpy().astype(np.float64)
+    assert np.abs(ff.sum(axis=0)).max() <= 1e-3 * np.abs(ff).max()
+    ctx.close()
