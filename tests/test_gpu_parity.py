@@ -352,3 +352,60 @@ def test_large_box_is_periodic_replication(pkg):
     ff = f[0].cpu().numpy().astype(np.float64)
     assert np.abs(ff.sum(axis=0)).max() <= 1e-3 * np.abs(ff).max()
     ctx.close()
+
+
+@pytest.mark.gpu
+def test_wide_capacity_takes_the_ballot_path_of_the_staged_scan(pkg):
+    """max_radial_nbrs = 256 does not fit the 8-bit packed slot fields: k_nbr compacts with ballots from the
+    staged stencil instead; results must not change."""
+    w = make_workload("C3")
+    pos, sp, g = _dev(w)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, max_radial_nbrs=256)
+    aev = ctx.aev_forward(pos, sp, w.box)
+    f = ctx.aev_backward(g)
+    ctx.check_status()
+    for which, rc in ((0, w.params.rcr), (1, w.params.rca)):
+        got = ctx.aev_export_pairs(which, cap=w.n_atoms * 40)
+        np.testing.assert_array_equal(got, _oracle_pairs(w, float(rc)))
+    want_a = oracle.aev_forward(w.params, w.pos, w.species, w.box, use_cells=True)
+    want_f = oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=True)
+    assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+    assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    ctx.close()
+
+
+@pytest.mark.gpu
+def test_cuda_graph_replay_with_new_positions(pkg):
+    """One evaluation captured in a CUDA graph and replayed after the positions changed in place (the MD-loop
+    calling pattern): no host-side state may be baked into the capture."""
+    w = make_workload("C2")
+    pos, sp, g = _dev(w)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch)
+    aev = torch.empty_like(g)
+    f = torch.empty((w.batch, w.n_atoms, 3), dtype=torch.float32, device="cuda")
+
+    def step():
+        ctx.aev_forward(pos, sp, w.box, aev_out=aev)
+        ctx.aev_backward(g, forces_out=f)
+
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        step()
+    # conformers in reverse order, written into the captured buffers
+    pos2 = np.ascontiguousarray(w.pos[::-1])
+    pos.copy_(torch.from_numpy(pos2).cuda())
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    ctx.check_status()
+    want_a = oracle.aev_forward(w.params, pos2, w.species, None)
+    want_f = oracle.aev_backward(w.params, pos2, w.species, None, w.grad_aev)
+    assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+    assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    del graph
+    ctx.close()
