@@ -32,6 +32,7 @@ struct DevParams {
     float shf_r[kNR];
     float shf_a[kNA];
     float cz[kNZ], sz[kNZ];      // cos / sin of the angle shifts
+    unsigned long long half2, neta_r2;                 // (0.5, 0.5) and (-eta_r log2 e) twice
     unsigned long long nshf_r2[kNR / 2];               // -shf_r, packed pairs (m even | m odd << 32)
     unsigned long long hcz2[kNZ / 2], hsz2[kNZ / 2];   // cos/2, sin/2 of the angle shifts, packed pairs (z even | z odd << 32)
 };
