@@ -132,7 +132,7 @@ def _work_counts(counts: np.ndarray, pos: np.ndarray, box, rcr: float):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on C4, from the one `ncu --set full` capture
 # summarised in profiles/r1_final_ncu_full.md (bench.py never runs under a profiler itself)
-NCU_TRAFFIC_BYTES = {"backward": 61.2e6 + 0.22e6, "aev": 25.4e6 + 0.32e6, "nbr": 0.96e6 + 0.19e6}
+NCU_TRAFFIC_BYTES = {"backward": 61.2e6 + 0.22e6, "aev": 25.4e6 + 0.42e6, "nbr": 0.96e6 + 0.18e6}
 
 
 def _flops(wc):
