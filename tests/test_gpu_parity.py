@@ -409,3 +409,22 @@ def test_cuda_graph_replay_with_new_positions(pkg):
     assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
     del graph
     ctx.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("zeta", [8.0, 16.0])
+def test_other_power_of_two_zeta(pkg, zeta):
+    """zeta != 32 takes the run-time squaring-chain instantiations of k_aev / k_backward."""
+    import dataclasses
+    w = make_workload("C2")
+    p = dataclasses.replace(w.params, zeta=np.float32(zeta))
+    pos, sp, g = _dev(w)
+    ctx = pkg.Context(p, max_atoms=w.n_atoms, max_batch=w.batch)
+    aev = ctx.aev_forward(pos, sp, w.box)
+    f = ctx.aev_backward(g)
+    ctx.check_status()
+    want_a = oracle.aev_forward(p, w.pos, w.species, None)
+    want_f = oracle.aev_backward(p, w.pos, w.species, None, w.grad_aev)
+    assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+    assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    ctx.close()
