@@ -167,7 +167,8 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
     extern __shared__ __align__(1024) unsigned char sm[];
     __shared__ int s_row[kTM];
     pdl_trigger();
-    pdl_wait();               // the AEV rows (k_aev) are complete
+    // everything up to the first AEV load runs before griddepcontrol.wait: the species partition (k_group) was
+    // complete before k_bin started, the weights are static, TMEM and barriers are this CTA's own
     const int s = blockIdx.y;
     const int rows = sp_count[s];
     const int r0 = blockIdx.x * kTM;
@@ -234,8 +235,9 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
             const int pieces = (kw / 8) * N1;
             for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
         };
-        F8 x0 = load_a(0), x1 = load_a(1);
         load_w0(0);
+        pdl_wait();              // the AEV rows (k_aev) are complete
+        F8 x0 = load_a(0), x1 = load_a(1);
         for (int kc = 0; kc < nkc; ++kc) {
             const int b = kc & 1;
             const int kw = min(kKC, K0 - kc * kKC);
