@@ -116,9 +116,10 @@ int aev_forward(aev_ctx *c, const float *pos, const int32_t *species, const floa
  *   grad_aev    device f32 [batch][n_atoms][L]  upstream dE/dAEV
  *   forces_out  device f32 [batch][n_atoms][3], OVERWRITTEN,
  *               forces_out[a] = - sum_i sum_slot grad_aev[i][slot]*dAEV[i][slot]/dx_a
- * The centre's own terms are reduced with warp shuffles; the gradient on each angular
- * neighbour is added with one fp32 RED per component, so forces are reproducible to
- * rounding, not bit for bit (the AEV itself is bit-reproducible).
+ * The centre's own terms are reduced with warp shuffles; the reaction on each radial
+ * neighbour and the gradient on each angular neighbour are added with one fp32 RED per
+ * component, so forces are reproducible to rounding, not bit for bit (the AEV itself is
+ * bit-reproducible while a cell's stencil fits the shared-memory stage, 1024 candidates).
  * AEV_ERR_STATE if no forward precedes it.  Asynchronous.
  */
 int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *stream);
