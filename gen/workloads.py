@@ -278,18 +278,27 @@ def _rotations(rng, m: int) -> np.ndarray:
     return rot
 
 
-def make_water_box(n_waters: int, side: float, seed: int, name: str,
+def make_water_box(n_waters: int, side, seed: int, name: str,
                    cos_scale: float = 1.0) -> Workload:
-    """Rigid waters (O-H 0.9572 A, HOH 104.52 deg) on a jittered partially filled cubic
-    lattice, random orientations, cubic periodic box (BASELINE.json:configs[2,3]).
+    """Rigid waters (O-H 0.9572 A, HOH 104.52 deg) on a jittered partially filled
+    lattice, random orientations, periodic box (BASELINE.json:configs[2,3]).  `side` is one
+    edge length (cubic box, the recipe of C3/C4) or three (orthorhombic box, PAPER.md:223:
+    the lattice then has ceil(L_k / (V/n)^(1/3)) sites along edge k).
     Atom order O,H,H per molecule; species O=3, H=0 (G7: S=4 everywhere).  Molecules are
     kept whole, so some H lie slightly outside [0,L) (G16)."""
     p = ani1x_style_params(cos_scale)
     rng = np.random.default_rng(seed)
-    n = int(math.ceil(n_waters ** (1.0 / 3.0) - 1e-9))
-    spacing = side / n
-    sites = rng.permutation(n ** 3)[:n_waters]
-    ix, iy, iz = sites // (n * n), (sites // n) % n, sites % n
+    if np.ndim(side) == 0:
+        n = int(math.ceil(n_waters ** (1.0 / 3.0) - 1e-9))
+        nk = np.array([n, n, n])
+        sides = np.array([float(side)] * 3)
+    else:
+        sides = np.asarray(side, dtype=np.float64).reshape(3)
+        s0 = (sides.prod() / n_waters) ** (1.0 / 3.0)
+        nk = np.ceil(sides / s0 - 1e-9).astype(np.int64)
+    spacing = sides / nk
+    sites = rng.permutation(int(nk.prod()))[:n_waters]
+    ix, iy, iz = sites // (nk[1] * nk[2]), (sites // nk[2]) % nk[1], sites % nk[2]
     centre = (np.stack([ix, iy, iz], axis=1) + 0.5) * spacing
 
     def place(m):
@@ -298,7 +307,7 @@ def make_water_box(n_waters: int, side: float, seed: int, name: str,
         return jit, np.einsum("mij,aj->mai", rot, _WATER)
 
     jit, rel = place(n_waters)
-    box = np.array([side] * 3, dtype=np.float32)
+    box = sides.astype(np.float32)
     mol_id = np.repeat(np.arange(n_waters), 3)
     for _ in range(100):
         pos = ((centre + jit)[:, None, :] + rel).reshape(-1, 3).astype(np.float32)

@@ -38,8 +38,11 @@
  *     capability 10.x gives AEV_ERR_UNSUPPORTED.
  *
  * Supported parameter space (else AEV_ERR_UNSUPPORTED): 1 <= num_species <= 8,
- * n_shf_r == 16, n_shf_a == 4, n_shf_z == 8 (the ANI-1x/2x shapes, BASELINE.json:configs[0]),
- * zeta a power of two in [1,64], 0 < rca <= rcr, 0 < cos_scale <= 1, orthorhombic boxes.
+ * n_shf_r == 16, n_shf_a == 4, n_shf_z == 8 (the shift counts of BASELINE.json:configs[0],
+ * "ANI-1x-style"; the lane mappings of the kernels are built on 16 / 4 x 8 = 32), zeta a power
+ * of two in [1,64], 0 < rca <= rcr, 0 < cos_scale <= 1; periodic boxes are orthorhombic (three
+ * edge lengths) or, with AEV_FLAG_TRICLINIC, reduced triclinic (three lattice vectors), every
+ * perpendicular width >= 2*rcr.
  */
 #ifndef AEV_B200_H
 #define AEV_B200_H
@@ -63,6 +66,18 @@ enum {
 
 typedef struct aev_ctx aev_ctx; /* opaque; owns all device workspace */
 
+/* aev_params.flags */
+enum {
+    AEV_FLAG_DETERMINISTIC = 1, /* aev_backward accumulates the force contributions on neighbours in
+                                   64-bit fixed point (2^-32 force units) instead of fp32 REDs: forces
+                                   are bit-identical run to run; a little slower  */
+    AEV_FLAG_MLP_FP32 = 2,      /* debugging: run the fp32 CUDA-core MLP kernel even where the tcgen05
+                                   kernel qualifies                                                     */
+    AEV_FLAG_TRICLINIC = 4      /* every `box` argument is HOST f32[9]: lattice vectors a, b, c as rows,
+                                   in reduced form a = (ax,0,0), b = (bx,by,0), c = (cx,cy,cz) with
+                                   ax, by, cz > 0, |bx| <= ax/2, |cx| <= ax/2, |cy| <= by/2             */
+};
+
 typedef struct {
     int32_t num_species;        /* S; species ids are 0..S-1, id < 0 marks a padding atom       */
     float rcr, rca;             /* radial / angular cutoff, same length unit as positions       */
@@ -80,6 +95,14 @@ typedef struct {
     int32_t max_radial_nbrs;    /* per-atom capacity for r < rcr (0 = default 128)              */
     int32_t max_angular_nbrs;   /* per-atom capacity for r < rca (0 = default 48; <= 64)        */
     int32_t device;             /* CUDA ordinal                                                 */
+    uint32_t flags;             /* AEV_FLAG_* bits, 0 = defaults                                */
+    float skin;                 /* Verlet skin (same length unit). 0 = the neighbour structure is
+                                   rebuilt in every aev_forward (reading G18, the headline protocol).
+                                   > 0: lists are built with cutoffs rcr+skin / rca+skin and reused by
+                                   later calls with the same shapes until some atom has moved more than
+                                   skin/2 since the build (checked on the device, CUDA-graph safe); the
+                                   exact cutoffs are applied when the lists are read, so results do
+                                   not depend on when the last rebuild happened (to rounding order).   */
 } aev_params;
 
 /* Creates a context (allocates workspace for max_batch*max_atoms atoms on `device`). Syncs. */
@@ -118,9 +141,10 @@ int aev_forward(aev_ctx *c, const float *pos, const int32_t *species, const floa
  *               forces_out[a] = - sum_i sum_slot grad_aev[i][slot]*dAEV[i][slot]/dx_a
  * The centre's own terms are reduced with warp shuffles; the reaction on each radial
  * neighbour and the gradient on each angular neighbour are added with one fp32 RED per
- * component, so forces are reproducible to rounding, not bit for bit (the AEV itself is
- * bit-reproducible while a cell's stencil fits the shared-memory stage, 1024 candidates).
- * AEV_ERR_STATE if no forward precedes it.  Asynchronous.
+ * component, so by default forces are reproducible to rounding, not bit for bit; with
+ * AEV_FLAG_DETERMINISTIC they are accumulated in 64-bit fixed point and are bit-identical
+ * run to run (the AEV itself always is while a cell's stencil fits the shared-memory stage,
+ * 1024 candidates).  AEV_ERR_STATE if no forward precedes it.  Asynchronous.
  */
 int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *stream);
 
@@ -129,12 +153,29 @@ int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *str
  *   dims     HOST i32 [n_layers+1]; dims[0] must equal L, dims[n_layers] must be 1,
  *            2 <= n_layers <= 4, hidden widths multiples of 16 and <= 256
  *   weights  HOST array of n_layers HOST pointers, layer l is f32 [dims[l]][dims[l+1]]
- *            row-major ("[in][out]"); weights are used as their bf16 hi+lo split
+ *            row-major ("[in][out]")
  *   biases   HOST array of n_layers HOST pointers, f32 [dims[l+1]]
  * Hidden activations are CELU(alpha); the last layer is linear.  Syncs.
+ * Which kernel runs: hidden widths <= 160 with the pre-activations of all hidden layers fitting
+ * 512 TMEM columns take the tcgen05 kernel (activations AND weights as bf16 hi + lo operands:
+ * hi*hi + lo*hi + hi*lo, fp32 accumulate; the weight-lo MMA is skipped for a network whose
+ * weights are all bf16-representable); other shapes run the fp32 CUDA-core kernel.
+ * ani_mlp_load == ani_mlp_load_model with model = 0 of an ensemble of 1.
  */
 int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const int32_t *dims,
                  const float *const *weights, const float *const *biases, float celu_alpha);
+
+/*
+ * Ensemble of networks over one AEV ("ANI-2x ... is an ensemble of eight models").
+ * ani_mlp_set_ensemble declares n_models (1..8) and drops every loaded network;
+ * ani_mlp_load_model loads the network of (model, species); all models of one species must have
+ * the same dims.  With an ensemble, ani_energy_forces returns the MEAN over the models of the
+ * energy and of dE/dAEV (one AEV forward, one AEV backward).  Sync.
+ */
+int ani_mlp_set_ensemble(aev_ctx *c, int32_t n_models);
+int ani_mlp_load_model(aev_ctx *c, int32_t model, int32_t species, int32_t n_layers,
+                       const int32_t *dims, const float *const *weights,
+                       const float *const *biases, float celu_alpha);
 
 /*
  * The whole path: neighbours + AEV + per-species MLP forward/backward + AEV backward.

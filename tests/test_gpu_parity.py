@@ -3,7 +3,8 @@ seeded inputs (BASELINE.json:north_star tolerances, written out below).
 
   neighbour pair sets ........ bit-exact (sorted (i<j) arrays equal)
   AEV ........................ max-abs error <= 1e-5 * max|AEV|
-  forces (fp32) .............. relative RMS error <= 1e-4
+  forces (fp32) .............. relative RMS error <= 1e-4, and every component within
+                               FORCE_MAX_TOL * max|F| (an error confined to a few atoms cannot hide in the norm)
   C5 energy+forces ........... forces relative RMS <= 1e-3 (bf16-split GEMMs, fp32 accumulate)
 """
 import numpy as np
@@ -20,6 +21,10 @@ pytestmark = pytest.mark.gpu
 AEV_TOL = 1e-5       # max-abs relative to max|AEV|          (north_star)
 FORCE_TOL = 1e-4     # relative RMS, fp32                     (north_star)
 C5_FORCE_TOL = 1e-3  # relative RMS with bf16 GEMMs           (BASELINE.json:configs[4])
+# per-component bound relative to max|F| (DESIGN.md section 6 lists the measured values: fp32 gives ~1e-6
+# on C1-C4; the bound leaves a decade of headroom and is still 10x below what one wrong atom would produce)
+FORCE_MAX_TOL = 2e-5
+C5_FORCE_MAX_TOL = 2e-4
 
 
 @pytest.fixture(scope="module")
@@ -39,6 +44,17 @@ def _dev(w):
 
 def _rel_rms(a, b):
     return float(np.sqrt(((a - b) ** 2).sum() / (b ** 2).sum()))
+
+
+def _check_forces(f, want, rms_tol=FORCE_TOL, max_tol=FORCE_MAX_TOL, what=""):
+    """north_star's relative-RMS bound plus a per-component max-abs bound relative to max|F|."""
+    f = np.asarray(f, dtype=np.float64)
+    rms = _rel_rms(f, want)
+    assert rms <= rms_tol, (what, "rel rms", rms)
+    worst = float(np.abs(f - want).max() / np.abs(want).max())
+    print("PARITY forces %s rel_rms %.3e max_abs_over_maxF %.3e" % (what, rms, worst))
+    assert worst <= max_tol, (what, "max abs / max|F|", worst)
+    return rms, worst
 
 
 def _oracle_pairs(w, rc):
@@ -81,8 +97,7 @@ def test_aev_and_forces_match_oracle(pkg, name, cos_scale):
     want_f = oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=uc)
     err = np.abs(aev - want_aev).max() / np.abs(want_aev).max()
     assert err <= AEV_TOL, (name, cos_scale, err)
-    rms = _rel_rms(forces, want_f)
-    assert rms <= FORCE_TOL, (name, cos_scale, rms)
+    _check_forces(forces, want_f, what=(name, cos_scale))
     # zero net force per system (north_star), relative to the force scale
     net = np.abs(forces.sum(axis=1)).max()
     assert net <= 1e-3 * np.sqrt((forces ** 2).mean()) * np.sqrt(w.n_atoms), net
@@ -143,7 +158,7 @@ def test_padding_atoms_and_tiny_systems(pkg):
     want = oracle.aev_forward(p, pos, sp, None)
     want_f = oracle.aev_backward(p, pos, sp, None, g)
     assert np.abs(aev - want).max() <= AEV_TOL * np.abs(want).max()
-    assert _rel_rms(f, want_f) <= FORCE_TOL
+    _check_forces(f, want_f)
     assert np.all(aev[0, 24:] == 0) and np.all(aev[1, :8] == 0)
     assert np.all(f[0, 24:] == 0) and np.all(f[1, :8] == 0)
     # one atom, two atoms: empty / single-pair environments
@@ -228,7 +243,7 @@ def test_c5_energy_and_forces(pkg):
     e, f = e.cpu().numpy(), f.cpu().numpy().astype(np.float64)
     we, wf, _ = oracle.energy_forces(w.params, w.pos, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
     assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
-    assert _rel_rms(f, wf) <= C5_FORCE_TOL
+    _check_forces(f, wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL)
     e2, f2 = ctx.ani_energy_forces_host(w.pos, w.species, w.box)
     assert abs(e2[0] - e[0]) <= 1e-9 * max(1.0, abs(e[0]))
     np.testing.assert_allclose(f2, f, rtol=0, atol=1e-5 * np.abs(f).max())   # RED order
@@ -252,7 +267,7 @@ def test_mlp_fp32_path_for_weights_that_are_not_bf16(pkg):
     e, f = e.cpu().numpy(), f.cpu().numpy().astype(np.float64)
     we, wf, _ = oracle.energy_forces(w.params, w.pos, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
     assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
-    assert _rel_rms(f, wf) <= FORCE_TOL
+    _check_forces(f, wf)
     ctx.close()
 
 
@@ -269,7 +284,7 @@ def test_mlp_tensor_core_path_other_depths(pkg):
     e, f = e.cpu().numpy(), f.cpu().numpy().astype(np.float64)
     we, wf, _ = oracle.energy_forces(w.params, w.pos, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
     assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
-    assert _rel_rms(f, wf) <= C5_FORCE_TOL
+    _check_forces(f, wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL)
     ctx.close()
 
 
@@ -291,7 +306,7 @@ def test_large_gas_phase_cluster_uses_the_unstaged_scan(pkg):
     want_f = oracle.aev_backward(wb.params, wb.pos, wb.species, None, wb.grad_aev, use_cells=False)
     a = aev.cpu().numpy().astype(np.float64)
     assert np.abs(a - want_aev).max() / np.abs(want_aev).max() <= AEV_TOL
-    assert _rel_rms(forces.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    _check_forces(forces.cpu().numpy().astype(np.float64), want_f)
     ctx.close()
 
 
@@ -318,7 +333,7 @@ def test_seven_species_ani2x_shape(pkg):
         want_a = oracle.aev_forward(p7, w.pos, sp, w.box, use_cells=w.box is not None)
         want_f = oracle.aev_backward(p7, w.pos, sp, w.box, g, use_cells=w.box is not None)
         assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
-        assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+        _check_forces(f.cpu().numpy().astype(np.float64), want_f)
         ctx.close()
 
 
@@ -370,7 +385,7 @@ def test_wide_capacity_takes_the_ballot_path_of_the_staged_scan(pkg):
     want_a = oracle.aev_forward(w.params, w.pos, w.species, w.box, use_cells=True)
     want_f = oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=True)
     assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
-    assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    _check_forces(f.cpu().numpy().astype(np.float64), want_f)
     ctx.close()
 
 
@@ -406,7 +421,7 @@ def test_cuda_graph_replay_with_new_positions(pkg):
     want_a = oracle.aev_forward(w.params, pos2, w.species, None)
     want_f = oracle.aev_backward(w.params, pos2, w.species, None, w.grad_aev)
     assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
-    assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    _check_forces(f.cpu().numpy().astype(np.float64), want_f)
     del graph
     ctx.close()
 
@@ -426,5 +441,5 @@ def test_other_power_of_two_zeta(pkg, zeta):
     want_a = oracle.aev_forward(p, w.pos, w.species, None)
     want_f = oracle.aev_backward(p, w.pos, w.species, None, w.grad_aev)
     assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
-    assert _rel_rms(f.cpu().numpy().astype(np.float64), want_f) <= FORCE_TOL
+    _check_forces(f.cpu().numpy().astype(np.float64), want_f)
     ctx.close()

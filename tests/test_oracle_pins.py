@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 import oracle
-from gen import ani1x_style_params, make_c1, make_c3
+from gen import ani1x_style_params, make_c1, make_c3, make_water_box
 
 from conftest import read_golden
 
@@ -173,6 +173,41 @@ def test_pairs_brute_vs_cell_vs_kdtree():
         np.testing.assert_array_equal(brute, kd.astype(np.int32))
     # statistics SURVEY.md section 8(d) recorded for this recipe: ~59.3 radial neighbours/atom
     assert 2 * len(oracle.pairs(pos, None, box, 5.2, "cell")) / 4500 == pytest.approx(59.3, abs=1.0)
+
+
+def test_cell_list_on_a_non_cubic_box():
+    """The cell-list path (the checker of C3/C4 and the timed CPU baseline) on an orthorhombic box
+    whose edges give three DIFFERENT cell counts (16 x 22 x 27.5 A -> 3 x 4 x 5 cells at 5.2 A, 4 x 6 x 7
+    at 3.5 A), atoms pushed outside [0, L): an x/y/z mix-up in the cell index or its decode fails here.
+    Pinned against the O(N^2) loop, scipy's periodic cKDTree and, for the featurizer and its gradient,
+    the brute-force result."""
+    from scipy.spatial import cKDTree
+    w = make_water_box(320, (16.0, 22.0, 27.5), 500, "ortho")
+    box = w.box
+    assert [int(np.floor(float(b) / 5.2)) for b in box] == [3, 4, 5]
+    rng = np.random.default_rng(11)
+    pos = (w.pos[0] + (rng.integers(-2, 3, size=w.pos[0].shape) * box)).astype(np.float32)
+    for rc in (5.2, 3.5):
+        brute = oracle.pairs(pos, w.species[0], box, rc, "brute")
+        cell = oracle.pairs(pos, w.species[0], box, rc, "cell")
+        np.testing.assert_array_equal(brute, cell)
+        b = box.astype(np.float64)
+        p64 = pos.astype(np.float64)
+        wrapped = p64 - b * np.floor(p64 / b)
+        wrapped = np.where(wrapped >= b, wrapped - b, wrapped)
+        kd = cKDTree(wrapped, boxsize=b).query_pairs(float(np.float32(rc)) - 1e-6, output_type="ndarray")
+        kd = np.sort(kd, axis=1)
+        kd = kd[np.lexsort((kd[:, 1], kd[:, 0]))]
+        # image shifts of up to two box lengths move float32 coordinates by ~1e-6 A: the generator's
+        # 1e-4 A cutoff margin keeps the pair set unchanged
+        np.testing.assert_array_equal(brute, kd.astype(np.int32))
+    a_b = oracle.aev_forward(w.params, pos[None], w.species, box, use_cells=False)
+    a_c = oracle.aev_forward(w.params, pos[None], w.species, box, use_cells=True)
+    np.testing.assert_array_equal(a_b, a_c)
+    f_b = oracle.aev_backward(w.params, pos[None], w.species, box, w.grad_aev, use_cells=False)
+    f_c = oracle.aev_backward(w.params, pos[None], w.species, box, w.grad_aev, use_cells=True)
+    np.testing.assert_allclose(f_b, f_c, rtol=0, atol=1e-12 * np.abs(f_b).max())   # OpenMP summation order
+    assert np.abs(f_b.sum(axis=1)).max() < 1e-9 * np.abs(f_b).max() * w.n_atoms
 
 
 def test_pairs_padding_and_images():
@@ -369,3 +404,42 @@ def test_batch_is_independent_conformers():
     a_cut = oracle.aev_forward(w.params, w.pos[:, :20], w.species[:, :20], None)
     np.testing.assert_array_equal(a_pad[0, :20], a_cut[0])
     assert np.all(a_pad[0, 20:] == 0.0)
+
+
+# ----------------------------------------------------------------------------- the cone point (G2)
+def _line3():
+    pos = np.array([[[0.0, 0.0, 0.0], [1.3, 0.0, 0.0], [2.9, 0.0, 0.0]]], dtype=np.float32)
+    return pos, np.array([[1, 3, 0]], dtype=np.int32)
+
+
+def test_collinear_triplet_damped_angle_matches_autograd():
+    """Exactly collinear j-i-k with c = 0.95: a regular point, so torch autograd of the independent
+    restatement pins the oracle's value and gradient there (cos = -1 for the middle atom, +1 for the ends)."""
+    import torch
+    pos, sp = _line3()
+    g = np.random.default_rng(6).standard_normal((1, 3, 384)).astype(np.float32)
+    x = torch.tensor(pos[0].astype(np.float64), requires_grad=True)
+    aev_t = _torch_aev(x, sp[0], P095)
+    (aev_t * torch.tensor(g[0].astype(np.float64))).sum().backward()
+    np.testing.assert_allclose(oracle.aev_forward(P095, pos, sp, None)[0], aev_t.detach().numpy(), rtol=1e-11, atol=1e-14)
+    np.testing.assert_allclose(oracle.aev_backward(P095, pos, sp, None, g)[0], -x.grad.numpy(), rtol=1e-9, atol=1e-11)
+    assert np.count_nonzero(aev_t.detach().numpy()[:, 64:]) > 0
+
+
+def test_collinear_triplet_literal_angle_cone_point():
+    """Exactly collinear j-i-k with c = 1 (the literal north_star formula): d(theta)/d(cos) is 0/0.
+    Reading G2 defines the perpendicular part of the gradient as 0.  What the mathematics fixes:
+    (a) by symmetry about the axis every force is along the line; (b) moving the atoms ALONG the line keeps
+    theta at 0 or pi, so E is smooth in those coordinates and central differences pin the axial forces;
+    (c) the value is the c -> 1 limit of the regular case."""
+    pos, sp = _line3()
+    g = np.random.default_rng(6).standard_normal((1, 3, 384)).astype(np.float32)
+    f = oracle.aev_backward(P100, pos, sp, None, g)[0]
+    assert np.all(np.isfinite(f))
+    assert np.all(f[:, 1:] == 0.0)
+    fd = _fd_forces(P100, pos, sp, None, g, [(0, 0), (1, 0), (2, 0)])
+    np.testing.assert_allclose(f[:, 0], fd, rtol=1e-5, atol=1e-7)
+    a1 = oracle.aev_forward(P100, pos, sp, None)
+    a2 = oracle.aev_forward(ani1x_style_params(1.0 - 1e-7), pos, sp, None)
+    # theta moves by sqrt(2e-7) = 4.5e-4 rad; zeta = 32 amplifies: a continuity check, not an identity
+    np.testing.assert_allclose(a1, a2, rtol=0, atol=1e-2 * np.abs(a1).max())
