@@ -16,6 +16,7 @@ from .workloads import (  # noqa: F401
     make_c3,
     make_c4,
     make_c5_weights,
+    make_ensemble_weights,
     make_workload,
     Workload,
 )

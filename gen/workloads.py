@@ -350,12 +350,14 @@ def _round_to_bf16(x: np.ndarray) -> np.ndarray:
     return u.astype(np.uint32).view(np.float32)
 
 
-def make_c5_weights(seed: int = 1, arch: Optional[Dict[int, List[int]]] = None
+def make_c5_weights(seed: int = 1, arch: Optional[Dict[int, List[int]]] = None, round_bf16: bool = True
                     ) -> Dict[int, Tuple[List[np.ndarray], List[np.ndarray]]]:
     """Random-init per-species MLPs (BASELINE.json:configs[4]): weights and biases
     ~ N(0, 1/fan_in) (variance; G13), draw order species H then O, layer 0..3, W then b,
     one default_rng(seed) stream.  W is [in][out] row-major float32, rounded to
-    bf16-representable values, which DEFINES the model (G14); biases stay float32."""
+    bf16-representable values, which DEFINES the model (G14); biases stay float32.
+    round_bf16=False keeps the float32 draws (a "trained-like" network whose weights are not
+    bf16-representable)."""
     arch = C5_ARCH if arch is None else arch
     rng = np.random.default_rng(seed)
     out = {}
@@ -366,10 +368,16 @@ def make_c5_weights(seed: int = 1, arch: Optional[Dict[int, List[int]]] = None
             std = dims[l] ** -0.5
             w = (rng.standard_normal((dims[l], dims[l + 1])) * std).astype(np.float32)
             b = (rng.standard_normal(dims[l + 1]) * std).astype(np.float32)
-            ws.append(_round_to_bf16(w))
+            ws.append(_round_to_bf16(w) if round_bf16 else w)
             bs.append(b)
         out[s] = (ws, bs)
     return out
+
+
+def make_ensemble_weights(n_models: int = 8, arch: Optional[Dict[int, List[int]]] = None, round_bf16: bool = True):
+    """An ensemble of `n_models` independently initialised networks per species (ANI-2x is
+    an ensemble of eight models): model m is make_c5_weights(seed = 1 + m)."""
+    return [make_c5_weights(seed=1 + m, arch=arch, round_bf16=round_bf16) for m in range(n_models)]
 
 
 # --------------------------------------------------------------------------- registry

@@ -173,6 +173,10 @@ int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const int32_t *d
  * energy and of dE/dAEV (one AEV forward, one AEV backward).  Sync.
  */
 int ani_mlp_set_ensemble(aev_ctx *c, int32_t n_models);
+/* Which kernel ani_energy_forces runs for the networks loaded so far: 1 = tcgen05 tensor-core kernel,
+ * 0 = fp32 CUDA-core kernel (a shape outside the envelope above, or AEV_FLAG_MLP_FP32),
+ * AEV_ERR_STATE = no network loaded. */
+int ani_mlp_kernel(const aev_ctx *c);
 int ani_mlp_load_model(aev_ctx *c, int32_t model, int32_t species, int32_t n_layers,
                        const int32_t *dims, const float *const *weights,
                        const float *const *biases, float celu_alpha);

@@ -206,6 +206,20 @@ def energy_forces(p, pos, species, box, nets: Dict[int, Tuple[List[np.ndarray], 
     return energy, forces, aev
 
 
+def energy_forces_ensemble(p, pos, species, box, models, alpha: float, use_cells: bool = False):
+    """Ensemble of networks over one AEV ("an ensemble of eight models"): `models` is a
+    list of `nets` dictionaries; the result is the plain mean over the models of `energy_forces`
+    (energy and forces are both linear in the per-model outputs).  Written as the definition:
+    one full evaluation per model, then the average."""
+    es, fs = [], []
+    aev = None
+    for nets in models:
+        e, f, aev = energy_forces(p, pos, species, box, nets, alpha, use_cells)
+        es.append(e)
+        fs.append(f)
+    return sum(es) / len(models), sum(fs) / len(models), aev
+
+
 def _backward_f64(p, pos, species, box, g64, use_cells):
     """aev_backward takes float32 g (the API's dtype).  For the full-model oracle the
     float64 g is split as hi(float32) + lo(float32); the backward is linear in g, so the

@@ -28,7 +28,7 @@ ERRORS = {
 
 EXPORTS = [
     "aev_create", "aev_destroy", "aev_length", "aev_neighbors", "aev_forward", "aev_backward",
-    "ani_mlp_load", "ani_energy_forces", "aev_forward_backward_host", "ani_energy_forces_host",
+    "ani_mlp_load", "ani_mlp_set_ensemble", "ani_mlp_load_model", "ani_mlp_kernel", "ani_energy_forces", "aev_forward_backward_host", "ani_energy_forces_host",
     "aev_export_pairs", "aev_export_counts", "aev_set_profiling", "aev_get_profile", "aev_status", "aev_launch_count", "aev_probe_fp32_tflops",
     "aev_error_string",
 ]
@@ -53,7 +53,12 @@ class _Params(C.Structure):
         ("max_atoms", C.c_int32), ("max_batch", C.c_int32),
         ("max_radial_nbrs", C.c_int32), ("max_angular_nbrs", C.c_int32),
         ("device", C.c_int32),
+        ("flags", C.c_uint32),
+        ("skin", C.c_float),
     ]
+
+
+AEV_FLAG_DETERMINISTIC, AEV_FLAG_MLP_FP32, AEV_FLAG_TRICLINIC = 1, 2, 4
 
 
 _lib = None
@@ -88,6 +93,13 @@ def lib():
         L.ani_mlp_load.restype = C.c_int
         L.ani_mlp_load.argtypes = [vp, i32, i32, C.POINTER(i32), C.POINTER(C.POINTER(C.c_float)),
                                    C.POINTER(C.POINTER(C.c_float)), C.c_float]
+        L.ani_mlp_set_ensemble.restype = C.c_int
+        L.ani_mlp_set_ensemble.argtypes = [vp, i32]
+        L.ani_mlp_load_model.restype = C.c_int
+        L.ani_mlp_load_model.argtypes = [vp, i32, i32, i32, C.POINTER(i32), C.POINTER(C.POINTER(C.c_float)),
+                                         C.POINTER(C.POINTER(C.c_float)), C.c_float]
+        L.ani_mlp_kernel.restype = C.c_int
+        L.ani_mlp_kernel.argtypes = [vp]
         L.ani_energy_forces.restype = C.c_int
         L.ani_energy_forces.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, vp, f32p, vp]
         L.aev_forward_backward_host.restype = C.c_int
@@ -146,7 +158,7 @@ class Context:
     """Owns one `aev_ctx`.  `params` is any object with the fields of gen.AniParams."""
 
     def __init__(self, params, max_atoms: int, max_batch: int = 1, device: int = 0,
-                 max_radial_nbrs: int = 0, max_angular_nbrs: int = 0):
+                 max_radial_nbrs: int = 0, max_angular_nbrs: int = 0, flags: int = 0, skin: float = 0.0):
         self._h = C.c_void_p()
         shf_r = np.ascontiguousarray(params.shf_r, dtype=np.float32)
         shf_a = np.ascontiguousarray(params.shf_a, dtype=np.float32)
@@ -157,7 +169,7 @@ class Context:
                     float(params.eta_a), float(params.zeta), len(shf_a), fp(shf_a),
                     len(shf_z), fp(shf_z), float(params.cos_scale),
                     int(max_atoms), int(max_batch), int(max_radial_nbrs), int(max_angular_nbrs),
-                    int(device))
+                    int(device), int(flags), float(skin))
         _check(lib().aev_create(C.byref(p), C.byref(self._h)), "aev_create")
         self.device = int(device)
         self.length = int(lib().aev_length(self._h))
@@ -204,16 +216,36 @@ class Context:
                "aev_backward")
         return forces_out
 
-    def ani_mlp_load(self, species: int, weights: Sequence[np.ndarray], biases: Sequence[np.ndarray],
-                     celu_alpha: float):
+    @staticmethod
+    def _net_args(weights, biases):
         ws = [np.ascontiguousarray(w, dtype=np.float32) for w in weights]
         bs = [np.ascontiguousarray(b, dtype=np.float32) for b in biases]
         dims = (C.c_int32 * (len(ws) + 1))(*([ws[0].shape[0]] + [w.shape[1] for w in ws]))
         fpp = C.POINTER(C.c_float)
         wp = (fpp * len(ws))(*[w.ctypes.data_as(fpp) for w in ws])
         bp = (fpp * len(bs))(*[b.ctypes.data_as(fpp) for b in bs])
+        return ws, bs, dims, wp, bp
+
+    def ani_mlp_load(self, species: int, weights: Sequence[np.ndarray], biases: Sequence[np.ndarray],
+                     celu_alpha: float):
+        ws, bs, dims, wp, bp = self._net_args(weights, biases)
         _check(lib().ani_mlp_load(self._h, int(species), len(ws), dims, wp, bp, float(celu_alpha)),
                "ani_mlp_load")
+
+    def mlp_kernel(self) -> str:
+        """'tcgen05' or 'fp32': the kernel ani_energy_forces runs for the loaded networks."""
+        rc = int(lib().ani_mlp_kernel(self._h))
+        _check(min(rc, 0), "ani_mlp_kernel")
+        return "tcgen05" if rc == 1 else "fp32"
+
+    def ani_mlp_set_ensemble(self, n_models: int):
+        _check(lib().ani_mlp_set_ensemble(self._h, int(n_models)), "ani_mlp_set_ensemble")
+
+    def ani_mlp_load_model(self, model: int, species: int, weights: Sequence[np.ndarray],
+                           biases: Sequence[np.ndarray], celu_alpha: float):
+        ws, bs, dims, wp, bp = self._net_args(weights, biases)
+        _check(lib().ani_mlp_load_model(self._h, int(model), int(species), len(ws), dims, wp, bp,
+                                        float(celu_alpha)), "ani_mlp_load_model")
 
     def ani_energy_forces(self, pos, species, box=None, energy_out=None, forces_out=None, stream=None):
         import torch

@@ -19,6 +19,7 @@ constexpr int kMaxS = 8;
 constexpr int kSpeciesShift = 26;  // neighbour entry .w = caller index of j | species << 26
 constexpr int kIdxMask = (1 << kSpeciesShift) - 1;
 constexpr int kMaxMlpLayers = 4;
+constexpr int kMaxModels = 8;      // networks per species in an ensemble
 
 // Everything the kernels need about the symmetry functions; passed by value (constant bank).
 struct DevParams {
@@ -59,6 +60,7 @@ struct Workspace {
     int4 *hdr;           // [n_total] per atom (caller order): (nA, nB, caller index, species)
     int *noff;           // [n_total][kMaxS+1] per-species list offsets: offA | offB << 16
     int *err;            // device error flags (bitmask)
+    long long *facc;     // [n_total][3] fixed-point force accumulator (AEV_FLAG_DETERMINISTIC), zero between calls
     unsigned *nbr_done;  // k_nbr CTAs that have read their bin counters (reset by the last one)
     unsigned long long *pair_count;  // export counter
 };
@@ -67,10 +69,12 @@ struct MlpNet {
     int loaded;
     int n_layers;
     int dims[kMaxMlpLayers + 1];
-    void *w_hi[kMaxMlpLayers];   // bf16 forward tensor-core operand  [in/8][out][8]   (ani_mlp_tc.cu)
-    void *w_lo[kMaxMlpLayers];   // bf16 backward tensor-core operand [out/8][in][8]
-    int bf16_exact;              // every hidden-layer weight is bf16-representable
-    int tc_ok;                   // shape + weights qualify for the tcgen05 kernel
+    // tensor-core operands (ani_mlp_tc.cu): bf16 hi part | bf16 residual part of every weight, chunked K-major
+    void *w_fwd[kMaxMlpLayers];  // forward operand  hi [in/8][out][8] | lo (same shape)
+    void *w_bwd[kMaxMlpLayers];  // backward operand hi [out/8][in][8] | lo
+    int bf16_exact;              // every hidden-layer weight is bf16-representable (the lo operands are all zero)
+    int tc_ok;                   // shape qualifies for the tcgen05 kernel
+    float alpha;                 // CELU alpha of this network
     float b_last;                // bias of the last (N = 1) layer
     float *w_f32[kMaxMlpLayers]; // f32 [in][out] as given
     float *w_t[kMaxMlpLayers];   // f32 [out][in] (transposed copy for the backward chain)
@@ -95,8 +99,8 @@ struct aev_ctx {
     size_t bwd_smem_optin, mlp_smem_optin;
     int tc_smem_optin;
     // MLP
-    aevb::MlpNet nets[aevb::kMaxS];
-    float celu_alpha;
+    aevb::MlpNet nets[aevb::kMaxModels][aevb::kMaxS];
+    int n_models;                // ensemble size (1 unless ani_mlp_set_ensemble was called)
     size_t mlp_cap;              // atoms the MLP workspaces are sized for
     float *mlp_aev;              // [n_total][L]   (ani_energy_forces workspace)
     float *mlp_grad;             // [n_total][L]
@@ -105,6 +109,7 @@ struct aev_ctx {
     int *sp_rows;                // [S][n_total] caller indices grouped by species
     int *sp_count;               // [S]
     void *tc_dev;                // device copy of the tensor-core network table (ani_mlp_tc.cu)
+    void *f32_dev;               // device copy of the fp32 network table (ani_mlp.cu)
     // host staging (pinned) + device staging for the *_host entry points
     int profiling;
     void *prof;                  // std::vector<ProfRec>* (aev_kernels.cu)
@@ -123,6 +128,22 @@ namespace aevb {
     } while (0)
 
 enum { kErrBitCapacity = 1, kErrBitState = 2 };
+
+// Every entry point runs on the context's device and leaves the caller's current device as it found it.
+class DeviceGuard {
+public:
+    explicit DeviceGuard(int dev) : prev_(-1), ok_(false)
+    {
+        if (cudaGetDevice(&prev_) != cudaSuccess) { prev_ = -1; return; }
+        ok_ = (prev_ == dev) || cudaSetDevice(dev) == cudaSuccess;
+        if (prev_ == dev) prev_ = -1;      // nothing to restore
+    }
+    ~DeviceGuard() { if (prev_ >= 0) cudaSetDevice(prev_); }
+    bool ok() const { return ok_; }
+private:
+    int prev_;
+    bool ok_;
+};
 
 // Programmatic dependent launch: a kernel launched with launch_pdl() may become resident while its
 // predecessor in the stream is still draining; it must pass pdl_wait() before it touches anything the

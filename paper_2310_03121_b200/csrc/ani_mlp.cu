@@ -3,7 +3,6 @@
 //   and the transposed chain dE/dAEV (BASELINE.json:configs[4]; DESIGN.md section 3 step 6).
 #include <cuda_bf16.h>
 #include <math.h>
-#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -20,8 +19,9 @@ struct MlpDev {
     const float *w[kMaxMlpLayers];
     const float *wt[kMaxMlpLayers];
     const float *b[kMaxMlpLayers];
+    float alpha;
 };
-struct MlpAll { MlpDev net[kMaxS]; };
+struct MlpAll { MlpDev net[kMaxModels][kMaxS]; };
 
 // Partition of the caller's atoms by species: sp_rows[s][0..sp_count[s]).  Slots are handed out
 // with one warp-aggregated atomic per (warp, species); the order inside a species is arbitrary
@@ -58,9 +58,9 @@ __device__ __forceinline__ float dcelu_from_h(float h, float inv_alpha)
 // v0: fp32 CUDA-core evaluation, TM rows per CTA, activations in shared memory.
 template <int TM>
 __global__ void __launch_bounds__(256)
-k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_rows,
-          const int *__restrict__ sp_count, const float *__restrict__ aev, float *__restrict__ grad,
-          double *__restrict__ energy, float alpha, int *__restrict__ err)
+k_mlp_f32(const MlpAll *__restrict__ M, int n_models, int L, int n_total, int n_atoms,
+          const int *__restrict__ sp_rows, const int *__restrict__ sp_count, const float *__restrict__ aev,
+          float *__restrict__ grad, double *__restrict__ energy, int *__restrict__ err)
 {
     extern __shared__ __align__(16) float sm[];
     pdl_trigger();
@@ -69,11 +69,15 @@ k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_
     const int rows = sp_count[s];
     const int r0 = blockIdx.x * TM;
     if (r0 >= rows) return;
-    const MlpDev &N = M.net[s];
+    __shared__ MlpDev N;      // network of (model blockIdx.z, species s)
+    if (threadIdx.x < sizeof(MlpDev) / 4)
+        reinterpret_cast<int *>(&N)[threadIdx.x] = reinterpret_cast<const int *>(&M->net[blockIdx.z][s])[threadIdx.x];
+    __syncthreads();
     if (!N.loaded) { if (threadIdx.x == 0) atomicOr(err, kErrBitState); return; }
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int nrow = min(TM, rows - r0);
-    const float inv_alpha = 1.0f / alpha;
+    const float alpha = N.alpha, inv_alpha = 1.0f / alpha;
+    const float inv_m = 1.0f / (float)n_models;      // ensemble: mean of the energies and of dE/dAEV
     const int nl = N.n_layers;
     __shared__ int s_row[TM];
     if (tid < TM) s_row[tid] = tid < nrow ? sp_rows[(size_t)s * n_total + r0 + tid] : -1;
@@ -127,7 +131,7 @@ k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_
             for (int k = lane; k < K; k += 32) acc = fmaf(h[nl - 1][r * K + k], W[k], acc);
 #pragma unroll
             for (int o = 16; o >= 1; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-            if (lane == 0) atomicAdd(&energy[s_row[r] / n_atoms], (double)(acc + N.b[nl - 1][0]));
+            if (lane == 0) atomicAdd(&energy[s_row[r] / n_atoms], (double)(acc + N.b[nl - 1][0]) * (double)inv_m);
         }
     }
     __syncthreads();   // the backward chain below overwrites h[nl-1] in place
@@ -167,7 +171,10 @@ k_mlp_f32(MlpAll M, int L, int n_total, int n_atoms, const int *__restrict__ sp_
             } else {
 #pragma unroll
                 for (int r = 0; r < TM; ++r)
-                    if (r < nrow) grad[(size_t)s_row[r] * L + k] = acc[r];
+                    if (r < nrow) {
+                        if (n_models == 1) grad[(size_t)s_row[r] * L + k] = acc[r];
+                        else atomicAdd(&grad[(size_t)s_row[r] * L + k], acc[r] * inv_m);      // grad was zeroed
+                    }
             }
         }
         __syncthreads();
@@ -181,16 +188,20 @@ namespace aevb {
 void mlp_tc_pack(const float *w, int K_in, int N_out, std::vector<__nv_bfloat16> &fwd, std::vector<__nv_bfloat16> &bwd,
                  bool *exact);
 
+static void free_net(MlpNet &n)
+{
+    for (int l = 0; l < kMaxMlpLayers; ++l) {
+        cudaFree(n.w_fwd[l]); cudaFree(n.w_bwd[l]); cudaFree(n.w_f32[l]); cudaFree(n.w_t[l]); cudaFree(n.bias[l]);
+    }
+    memset(&n, 0, sizeof(n));
+}
+
 void mlp_free(aev_ctx *c)
 {
-    for (int s = 0; s < kMaxS; ++s) {
-        MlpNet &n = c->nets[s];
-        for (int l = 0; l < kMaxMlpLayers; ++l) {
-            cudaFree(n.w_hi[l]); cudaFree(n.w_lo[l]); cudaFree(n.w_f32[l]); cudaFree(n.w_t[l]);
-            cudaFree(n.bias[l]);
-        }
-        memset(&n, 0, sizeof(n));
-    }
+    for (int m = 0; m < kMaxModels; ++m)
+        for (int s = 0; s < kMaxS; ++s) free_net(c->nets[m][s]);
+    cudaFree(c->f32_dev);
+    c->f32_dev = nullptr;
 }
 
 int mlp_group(aev_ctx *c, const int32_t *species, int n_total, int batch, double *energy_out, cudaStream_t st)
@@ -201,45 +212,58 @@ int mlp_group(aev_ctx *c, const int32_t *species, int n_total, int batch, double
     return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
 }
 
+// Device table of the fp32 kernel; rebuilt whenever a network is (re)loaded.  Syncs.
+static int mlp_f32_upload(aev_ctx *c)
+{
+    static MlpAll M;      // 8 KB: not on the stack
+    memset(&M, 0, sizeof(M));
+    for (int m = 0; m < c->n_models; ++m)
+        for (int s = 0; s < c->dp.S; ++s) {
+            const MlpNet &n = c->nets[m][s];
+            MlpDev &d = M.net[m][s];
+            d.loaded = n.loaded; d.n_layers = n.n_layers; d.alpha = n.alpha;
+            for (int l = 0; l <= n.n_layers; ++l) d.dims[l] = n.dims[l];
+            for (int l = 0; l < n.n_layers; ++l) { d.w[l] = n.w_f32[l]; d.wt[l] = n.w_t[l]; d.b[l] = n.bias[l]; }
+        }
+    if (!c->f32_dev) AEVB_CUDA(cudaMalloc(&c->f32_dev, sizeof(MlpAll)));
+    AEVB_CUDA(cudaMemcpy(c->f32_dev, &M, sizeof(MlpAll), cudaMemcpyHostToDevice));
+    return AEV_OK;
+}
+
 int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_atoms, int batch,
                          const float *aev, float *grad_aev, double *energy_out, cudaStream_t st)
 {
-    const int S = c->dp.S, L = c->dp.L;
-    MlpAll M;
-    memset(&M, 0, sizeof(M));
+    const int S = c->dp.S, L = c->dp.L, nm = c->n_models;
     int sum_hidden = 0;
-    for (int s = 0; s < S; ++s) {
-        const MlpNet &n = c->nets[s];
-        MlpDev &d = M.net[s];
-        d.loaded = n.loaded; d.n_layers = n.n_layers;
-        int sh = 0;
-        for (int l = 0; l <= n.n_layers; ++l) d.dims[l] = n.dims[l];
-        for (int l = 0; l < n.n_layers; ++l) {
-            d.w[l] = n.w_f32[l]; d.wt[l] = n.w_t[l]; d.b[l] = n.bias[l];
-            sh += n.dims[l];
+    bool all_tc = true;
+    for (int m = 0; m < nm; ++m)
+        for (int s = 0; s < S; ++s) {
+            const MlpNet &n = c->nets[m][s];
+            if (!n.loaded) continue;
+            int sh = 0;
+            for (int l = 0; l < n.n_layers; ++l) sh += n.dims[l];
+            if (sh > sum_hidden) sum_hidden = sh;
+            if (!n.tc_ok) all_tc = false;
         }
-        if (sh > sum_hidden) sum_hidden = sh;
-    }
-    constexpr int TM = 8;
-    const size_t smem = (size_t)TM * sum_hidden * sizeof(float);
-    if (smem > c->mlp_smem_optin) {
-        AEVB_CUDA(cudaFuncSetAttribute(k_mlp_f32<TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        c->mlp_smem_optin = smem;
-    }
     prof_begin(c, 5, st);
     // tensor-core path when every loaded network qualifies (ani_mlp_tc.cu); else fp32 CUDA cores
-    bool all_tc = true;
-    for (int s = 0; s < S; ++s)
-        if (c->nets[s].loaded && !c->nets[s].tc_ok) all_tc = false;
-    if (all_tc && !getenv("AEVB_MLP_FP32")) {
+    if (all_tc && !(c->hp.flags & AEV_FLAG_MLP_FP32)) {
         const int rc = mlp_tc_forward_backward(c, n_total, n_atoms, aev, grad_aev, energy_out, st);
         prof_end(c, st);
         c->launches += 1;
         return rc;
     }
-    dim3 grid((n_total + TM - 1) / TM, S);
-    launch_pdl(k_mlp_f32<TM>, grid, dim3(256), smem, st, M, L, n_total, n_atoms, c->sp_rows, c->sp_count, aev, grad_aev,
-               energy_out, c->celu_alpha, c->ws.err);
+    constexpr int TM = 8;
+    const size_t smem = (size_t)TM * sum_hidden * sizeof(float);
+    if (smem > 200 * 1024) return AEV_ERR_UNSUPPORTED;
+    if (smem > c->mlp_smem_optin) {
+        AEVB_CUDA(cudaFuncSetAttribute(k_mlp_f32<TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        c->mlp_smem_optin = smem;
+    }
+    if (!c->f32_dev) return AEV_ERR_STATE;
+    dim3 grid((n_total + TM - 1) / TM, S, nm);
+    launch_pdl(k_mlp_f32<TM>, grid, dim3(256), smem, st, static_cast<const MlpAll *>(c->f32_dev), nm, L, n_total, n_atoms,
+               (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->ws.err);
     prof_end(c, st);
     c->launches += 1;
     if (cudaGetLastError() != cudaSuccess) return AEV_ERR_CUDA;
@@ -248,11 +272,38 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
 
 }  // namespace aevb
 
-extern "C" int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const int32_t *dims,
-                            const float *const *weights, const float *const *biases, float celu_alpha)
+extern "C" int ani_mlp_kernel(const aev_ctx *c)
+{
+    if (!c) return AEV_ERR_INVALID_ARG;
+    bool any = false, all_tc = true;
+    for (int m = 0; m < c->n_models; ++m)
+        for (int s = 0; s < c->dp.S; ++s) {
+            const MlpNet &n = c->nets[m][s];
+            if (!n.loaded) continue;
+            any = true;
+            if (!n.tc_ok) all_tc = false;
+        }
+    if (!any) return AEV_ERR_STATE;
+    return (all_tc && !(c->hp.flags & AEV_FLAG_MLP_FP32)) ? 1 : 0;
+}
+
+extern "C" int ani_mlp_set_ensemble(aev_ctx *c, int32_t n_models)
+{
+    if (!c || n_models < 1 || n_models > kMaxModels) return AEV_ERR_INVALID_ARG;
+    DeviceGuard guard(c->device);
+    if (!guard.ok()) return AEV_ERR_CUDA;
+    AEVB_CUDA(cudaDeviceSynchronize());
+    for (int m = 0; m < kMaxModels; ++m)
+        for (int s = 0; s < kMaxS; ++s) free_net(c->nets[m][s]);
+    c->n_models = n_models;
+    return AEV_OK;
+}
+
+extern "C" int ani_mlp_load_model(aev_ctx *c, int32_t model, int32_t species, int32_t n_layers, const int32_t *dims,
+                                  const float *const *weights, const float *const *biases, float celu_alpha)
 {
     if (!c || !dims || !weights || !biases) return AEV_ERR_INVALID_ARG;
-    if (species < 0 || species >= c->dp.S) return AEV_ERR_INVALID_ARG;
+    if (species < 0 || species >= c->dp.S || model < 0 || model >= c->n_models) return AEV_ERR_INVALID_ARG;
     if (n_layers < 2 || n_layers > kMaxMlpLayers) return AEV_ERR_UNSUPPORTED;
     if (dims[0] != c->dp.L || dims[n_layers] != 1) return AEV_ERR_INVALID_ARG;
     if (!(celu_alpha > 0.f)) return AEV_ERR_INVALID_ARG;
@@ -260,15 +311,22 @@ extern "C" int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const
         if (dims[l] < 16 || dims[l] > 256 || dims[l] % 16) return AEV_ERR_UNSUPPORTED;
     for (int l = 0; l < n_layers; ++l)
         if (!weights[l] || !biases[l]) return AEV_ERR_INVALID_ARG;
-    AEVB_CUDA(cudaSetDevice(c->device));
-    AEVB_CUDA(cudaDeviceSynchronize());
-    MlpNet &n = c->nets[species];
-    for (int l = 0; l < kMaxMlpLayers; ++l) {
-        cudaFree(n.w_hi[l]); cudaFree(n.w_lo[l]); cudaFree(n.w_f32[l]); cudaFree(n.w_t[l]); cudaFree(n.bias[l]);
+    // all models of one species share one shape (one launch geometry per species)
+    for (int m = 0; m < c->n_models; ++m) {
+        const MlpNet &o = c->nets[m][species];
+        if (m == model || !o.loaded) continue;
+        if (o.n_layers != n_layers) return AEV_ERR_INVALID_ARG;
+        for (int l = 0; l <= n_layers; ++l)
+            if (o.dims[l] != dims[l]) return AEV_ERR_INVALID_ARG;
     }
-    memset(&n, 0, sizeof(n));
+    DeviceGuard guard(c->device);
+    if (!guard.ok()) return AEV_ERR_CUDA;
+    AEVB_CUDA(cudaDeviceSynchronize());
+    MlpNet &n = c->nets[model][species];
+    free_net(n);
     n.n_layers = n_layers;
     n.bf16_exact = 1;
+    n.alpha = celu_alpha;
     for (int l = 0; l <= n_layers; ++l) n.dims[l] = dims[l];
     for (int l = 0; l < n_layers; ++l) {
         const int K = dims[l], No = dims[l + 1];
@@ -282,18 +340,25 @@ extern "C" int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const
             for (int o = 0; o < No; ++o) wt[(size_t)o * K + k] = weights[l][(size_t)k * No + o];
         AEVB_CUDA(cudaMalloc((void **)&n.w_f32[l], cnt * 4));
         AEVB_CUDA(cudaMalloc((void **)&n.w_t[l], cnt * 4));
-        AEVB_CUDA(cudaMalloc(&n.w_hi[l], fw.size() * 2));
-        AEVB_CUDA(cudaMalloc(&n.w_lo[l], bw.size() * 2));
+        AEVB_CUDA(cudaMalloc(&n.w_fwd[l], fw.size() * 2));
+        AEVB_CUDA(cudaMalloc(&n.w_bwd[l], bw.size() * 2));
         AEVB_CUDA(cudaMalloc((void **)&n.bias[l], (size_t)No * 4));
         AEVB_CUDA(cudaMemcpy(n.w_f32[l], weights[l], cnt * 4, cudaMemcpyHostToDevice));
         AEVB_CUDA(cudaMemcpy(n.w_t[l], wt.data(), cnt * 4, cudaMemcpyHostToDevice));
-        AEVB_CUDA(cudaMemcpy(n.w_hi[l], fw.data(), fw.size() * 2, cudaMemcpyHostToDevice));
-        AEVB_CUDA(cudaMemcpy(n.w_lo[l], bw.data(), bw.size() * 2, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.w_fwd[l], fw.data(), fw.size() * 2, cudaMemcpyHostToDevice));
+        AEVB_CUDA(cudaMemcpy(n.w_bwd[l], bw.data(), bw.size() * 2, cudaMemcpyHostToDevice));
         AEVB_CUDA(cudaMemcpy(n.bias[l], biases[l], (size_t)No * 4, cudaMemcpyHostToDevice));
     }
     n.b_last = biases[n_layers - 1][0];
     n.tc_ok = mlp_tc_eligible(n, c->dp.L) ? 1 : 0;
     n.loaded = 1;
-    c->celu_alpha = celu_alpha;
+    int rc = mlp_f32_upload(c);
+    if (rc) return rc;
     return mlp_tc_upload(c);
+}
+
+extern "C" int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const int32_t *dims,
+                            const float *const *weights, const float *const *biases, float celu_alpha)
+{
+    return ani_mlp_load_model(c, 0, species, n_layers, dims, weights, biases, celu_alpha);
 }

@@ -5,9 +5,11 @@
 // (M = 128 rows, N = layer width, K = 16 per instruction) whose accumulator lives in TMEM:
 //   forward  z_l  = h_(l-1) W_l            A = activations (shared memory), B = W_l  [N=out][K=in]
 //   backward d_l' = d_(l+1) W_(l+1)^T      A = upstream    (shared memory), B = W^T  [N=in][K=out]
-// Activations are fp32 values split into two bf16 operands (hi + lo, error 2^-17); the weights
-// are the model's bf16-representable values (reading G14), so each GEMM is two MMAs
-// per K step.  The pre-activations z_l stay resident in TMEM between the forward and the
+// Activations and weights are fp32 values split into two bf16 operands each (hi + lo); every GEMM
+// is hi*hi + lo*hi + hi*lo per K step (the lo*lo term, 2^-18 relative, is dropped).  A network
+// whose weights are all bf16-representable (reading G14) has zero weight-lo operands
+// and skips the third MMA.  grid.z = model of an ensemble: every model reads the
+// same AEV tile and adds its share of the mean energy and of the mean dE/dAEV.  The pre-activations z_l stay resident in TMEM between the forward and the
 // backward sweep (CELU' is recomputed from them); bias, CELU, the last (N = 1) layer, the
 // energy sum and the bf16 split run in the epilogue, one thread per row (tcgen05.ld 32x32b).
 //
@@ -117,6 +119,11 @@ __device__ __forceinline__ void ldg256(const float *p, float *v)
                  : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
                  : "l"(p));
 }
+// 16-byte vector reduction (sm_90+): four fp32 adds in one request
+__device__ __forceinline__ void red_add_v4(float *p, const float *v)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]) : "memory");
+}
 __device__ __forceinline__ void stg256(float *p, const float *v)
 {
     asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]),
@@ -149,20 +156,22 @@ __device__ __forceinline__ float dcelu_tc(float x, float inv_alpha) { return x >
 
 struct TcNetDev {
     int loaded, nh;                      // nh = hidden layers (1..3); layer l maps dims[l] -> dims[l+1]
+    int need_lo;                         // some hidden-layer weight is not bf16-representable: third MMA per K step
+    float alpha;                         // CELU alpha
     int dims[kMaxMlpLayers + 1];         // dims[0] = L, dims[1..nh] hidden widths, dims[nh+1] = 1
-    const __nv_bfloat16 *wf[3];          // forward operand of layer l:  [K/8][N][8], K = dims[l],   N = dims[l+1]
-    const __nv_bfloat16 *wb[3];          // backward operand of layer l: [K/8][N][8], K = dims[l+1], N = dims[l]
+    const __nv_bfloat16 *wf[3];          // forward operand of layer l:  hi [K/8][N][8] | lo, K = dims[l],   N = dims[l+1]
+    const __nv_bfloat16 *wb[3];          // backward operand of layer l: hi [K/8][N][8] | lo, K = dims[l+1], N = dims[l]
     const float *bias[3];                // bias of layer l (width dims[l+1])
     const float *wlast;                  // last layer weights [dims[nh]]
     float blast;
     int zoff[3];                         // TMEM column of z_(l+1) = output of layer l
 };
-struct TcAll { TcNetDev net[kMaxS]; };
+struct TcAll { TcNetDev net[kMaxModels][kMaxS]; };
 
 __global__ void __launch_bounds__(kTcThreads, 1)
-k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const int *__restrict__ sp_rows,
-         const int *__restrict__ sp_count, const float *__restrict__ aev, float *__restrict__ grad,
-         double *__restrict__ energy, float alpha, int *__restrict__ err)
+k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_atoms,
+         const int *__restrict__ sp_rows, const int *__restrict__ sp_count, const float *__restrict__ aev,
+         float *__restrict__ grad, double *__restrict__ energy, int *__restrict__ err)
 {
     extern __shared__ __align__(1024) unsigned char sm[];
     __shared__ int s_row[kTM];
@@ -172,16 +181,20 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
     const int s = blockIdx.y;
     const int rows = sp_count[s];
     const int r0 = blockIdx.x * kTM;
-    if (r0 >= rows) return;
+    // (a CTA that leaves early still passes griddepcontrol.wait: completion of this grid must imply completion
+    //  of everything before it in the launch chain - aev_common.cuh)
+    if (r0 >= rows) { pdl_wait(); return; }
     __shared__ TcNetDev N;
     if (threadIdx.x < sizeof(TcNetDev) / 4)
-        reinterpret_cast<int *>(&N)[threadIdx.x] = reinterpret_cast<const int *>(&Mg->net[s])[threadIdx.x];
+        reinterpret_cast<int *>(&N)[threadIdx.x] = reinterpret_cast<const int *>(&Mg->net[blockIdx.z][s])[threadIdx.x];
     __syncthreads();
-    if (!N.loaded) { if (threadIdx.x == 0) atomicOr(err, kErrBitState); return; }
+    if (!N.loaded) { if (threadIdx.x == 0) atomicOr(err, kErrBitState); pdl_wait(); return; }
     const int tid = threadIdx.x, wid = tid >> 5;
     const int row = tid & (kTM - 1), grp = tid >> 7;     // epilogue: thread = (row, column group)
-    const float inv_alpha = 1.0f / alpha;
+    const float alpha = N.alpha, inv_alpha = 1.0f / alpha;
+    const float inv_m = 1.0f / (float)n_models;
     const int nh = N.nh;
+    const bool need_lo = N.need_lo != 0;
 
     unsigned char *act = sm;
     unsigned char *wbuf[2] = {sm + kActBytes, sm + kActBytes + kWBufBytes};
@@ -234,6 +247,11 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
             unsigned char *dst = wbuf[kc & 1];
             const int pieces = (kw / 8) * N1;
             for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
+            if (need_lo) {      // residual operand: second half of the stage buffer
+                const unsigned char *srcl = src + (size_t)((K0 + 7) / 8) * N1 * 16;
+                for (int t = tid; t < pieces; t += kTcThreads)
+                    cp_async16_tc(dst + kWBufBytes / 2 + t * 16, srcl + (size_t)t * 16);
+            }
         };
         load_w0(0);
         pdl_wait();              // the AEV rows (k_aev) are complete
@@ -262,6 +280,9 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
                     const unsigned long long bd = smem_desc(b_a + ks * 2 * N1 * 16, N1 * 16, 128);
                     umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 4096, 2048, 128), bd, idesc, (kc | ks) != 0);
                     umma_bf16(tmem + N.zoff[0], smem_desc(a_lo + ks * 4096, 2048, 128), bd, idesc, 1u);
+                    if (need_lo)
+                        umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 4096, 2048, 128),
+                                  smem_desc(b_a + kWBufBytes / 2 + ks * 2 * N1 * 16, N1 * 16, 128), idesc, 1u);
                 }
                 umma_commit(&bar[b]);
             }
@@ -282,13 +303,14 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
     }
 
     TC_STAMP(1);
-    // whole-layer weight operand -> shared memory (contiguous [K/8][N][8] block)
+    // whole-layer weight operand -> shared memory (contiguous [K/8][N][8] block; the residual operand right behind it)
     auto load_w = [&](const __nv_bfloat16 *w, int K, int Nn, unsigned char *dst) {
         const unsigned char *src = reinterpret_cast<const unsigned char *>(w);
-        const int pieces = (K / 8) * Nn;
+        const int pieces = (K / 8) * Nn * (need_lo ? 2 : 1);      // hi | lo are adjacent in global memory too
         for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
     };
-    // D[tmem + dcol] = act[128 x K] (hi + lo) * B[Nn x K]^T, issued by one thread, completion on bar[2]
+    // D[tmem + dcol] = act[128 x K] (hi + lo) * B[Nn x K]^T (hi [+ lo at wsm + K*Nn*2]), issued by one thread,
+    // completion on bar[2]
     auto gemm = [&](int K, int Nn, const unsigned char *wsm, int lbo_b, unsigned dcol) {
         if (tid == 0) {
             tc_fence_after();
@@ -298,6 +320,9 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
                 const unsigned long long bd = smem_desc(b_a + ks * 2 * lbo_b, lbo_b, 128);
                 umma_bf16(tmem + dcol, smem_desc(a_hi + ks * 4096, 2048, 128), bd, idesc, ks != 0);
                 umma_bf16(tmem + dcol, smem_desc(a_lo + ks * 4096, 2048, 128), bd, idesc, 1u);
+                if (need_lo)
+                    umma_bf16(tmem + dcol, smem_desc(a_hi + ks * 4096, 2048, 128),
+                              smem_desc(b_a + K * Nn * 2 + ks * 2 * lbo_b, lbo_b, 128), idesc, 1u);
             }
             umma_commit(&bar[2]);
         }
@@ -328,6 +353,9 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
         // z_l (output of layer l-1) is complete in TMEM at zoff[l-1]
         const int Nl = N.dims[l], ncl = Nl >> 3;
         const float *bl = N.bias[l - 1];
+        // (every earlier GEMM has completed here, so with residual operands - up to 80 KB, both buffers - the
+        //  operand always starts at wbuf[0])
+        if (need_lo) wsel = 0;
         if (l < nh) load_w(N.wf[l], Nl, N.dims[l + 1], wbuf[wsel]);               // overlaps the epilogue below
         else if (nh >= 2) load_w(N.wb[nh - 1], Nl, N.dims[nh - 1], wbuf[wsel]);
         float v[kMaxC][8];
@@ -370,7 +398,7 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
             wait_gemm();
         } else {
             // energy: one fp64 atomic per warp when its rows belong to one system (the usual case)
-            double ed = my_row >= 0 ? (double)e + (grp == 0 ? (double)N.blast : 0.0) : 0.0;
+            double ed = my_row >= 0 ? ((double)e + (grp == 0 ? (double)N.blast : 0.0)) * (double)inv_m : 0.0;
             const int bsys = my_row >= 0 ? my_row / n_atoms : -1;
             const unsigned have = __ballot_sync(0xffffffffu, my_row >= 0);
             if (have) {
@@ -394,9 +422,14 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
         const unsigned dcol = N.zoff[l];                   // z_(l+1) is dead: reuse its columns
         sync_for_mma();
         gemm(Kb, Nb, wbuf[wsel], Nb * 16, dcol);
-        wsel ^= 1;
-        if (l >= 2) load_w(N.wb[l - 1], Nb, N.dims[l - 1], wbuf[wsel]);   // next operand while the MMAs run
-        wait_gemm();
+        if (!need_lo) {
+            wsel ^= 1;
+            if (l >= 2) load_w(N.wb[l - 1], Nb, N.dims[l - 1], wbuf[wsel]);   // next operand while the MMAs run
+            wait_gemm();
+        } else {      // residual operands span both buffers: the next operand follows the GEMM
+            wait_gemm();
+            if (l >= 2) load_w(N.wb[l - 1], Nb, N.dims[l - 1], wbuf[0]);
+        }
         const float *bl = N.bias[l - 1];
 #pragma unroll
         for (int i = 0; i < kMaxC; ++i) {
@@ -417,30 +450,36 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
     }
 
     TC_STAMP(3);
-    // ------------------------------------------------------------------ d_0 = d_1 W_0^T, N = L in chunks of 128
+    // ------------------------------------------------------------------ d_0 = d_1 W_0^T, N = L in chunks of CW
     {
         const int Kb = N.dims[1];
-        const int nch = (L + 127) / 128;
+        const int CW = need_lo ? 64 : 128;       // a chunk's hi (+ lo) operand fits one 40 KB buffer
+        const int nch = (L + CW - 1) / CW;
+        const size_t lo_off = (size_t)((Kb + 7) / 8) * L * 16;
+        if (need_lo) wsel = 0;
         auto load_chunk = [&](int j, unsigned char *dst) {
-            const int n0 = j * 128, nw = min(128, L - n0);
+            const int n0 = j * CW, nw = min(CW, L - n0);
             const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wb[0]);
             const int pieces = (Kb / 8) * nw;
             for (int t = tid; t < pieces; t += kTcThreads) {
                 const int kc = t / nw, n = t - kc * nw;
                 cp_async16_tc(dst + t * 16, src + ((size_t)kc * L + n0 + n) * 16);
+                if (need_lo) cp_async16_tc(dst + Kb * nw * 2 + t * 16, src + lo_off + ((size_t)kc * L + n0 + n) * 16);
             }
         };
+        // accumulators alternate between two TMEM slots (every z is dead by now): chunk j at column (j & 1) * 128
         load_chunk(0, wbuf[wsel]);
         sync_for_mma();
-        gemm(Kb, min(128, L), wbuf[wsel], min(128, L) * 16, 0u);
+        gemm(Kb, min(CW, L), wbuf[wsel], min(CW, L) * 16, 0u);
         for (int j = 0; j < nch; ++j) {
-            const int n0 = j * 128, nw = min(128, L - n0);
+            const int n0 = j * CW, nw = min(CW, L - n0);
+            const unsigned slot = (unsigned)(j & 1) * 128u;
             if (j + 1 < nch) load_chunk(j + 1, wbuf[wsel ^ 1]);
             wait_gemm();
             if (j + 1 < nch) {
-                const int nw1 = min(128, L - (j + 1) * 128);
+                const int nw1 = min(CW, L - (j + 1) * CW);
                 sync_for_mma();
-                gemm(Kb, nw1, wbuf[wsel ^ 1], nw1 * 16, (unsigned)((j + 1) * 128));
+                gemm(Kb, nw1, wbuf[wsel ^ 1], nw1 * 16, slot ^ 128u);
                 wsel ^= 1;
             }
             // tcgen05.ld is warp-collective: rows without an atom take part, only the store is skipped
@@ -449,13 +488,25 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
                 const int c = grp + i * kTcGroups;
-                if (c * 8 < nw) tmem_ld8(tlane + n0 + c * 8, v[i]);
+                if (c * 8 < nw) tmem_ld8(tlane + slot + c * 8, v[i]);
             }
             tmem_wait();
+            // the epilogue of chunk j must have read its slot before the GEMM of chunk j+2 overwrites it: that GEMM is
+            // issued after the next iteration's sync_for_mma (a CTA-wide barrier behind this read)
+            tc_fence_before();
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
                 const int c = grp + i * kTcGroups;
-                if (c * 8 < nw && my_row >= 0) stg256(dst + c * 8, v[i]);
+                if (c * 8 < nw && my_row >= 0) {
+                    if (n_models == 1) {
+                        stg256(dst + c * 8, v[i]);
+                    } else {      // mean over the ensemble: grad was zeroed before the launch chain
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) v[i][k] *= inv_m;
+                        red_add_v4(dst + c * 8, v[i]);
+                        red_add_v4(dst + c * 8 + 4, v[i] + 4);
+                    }
+                }
             }
         }
     }
@@ -477,23 +528,24 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int L, int n_total, int n_atoms, const in
 namespace aevb {
 
 // Shapes the tensor-core kernel covers (everything else runs the fp32 CUDA-core kernel):
-// 1..3 hidden layers of width 16..160 (multiples of 16), L <= 512 (multiple of 16), weight
-// operands of the inner layers <= 40 KB, z_l and the backward accumulators fit 512 TMEM columns,
-// and every hidden-layer weight is bf16-representable (the model of reading G14).
+// 1..3 hidden layers of width 16..160 (multiples of 16), L a multiple of 16, the weight operand of
+// every inner layer within the shared-memory buffers (40 KB; 80 KB hi + lo for weights that are not
+// bf16-representable), z_l and the backward accumulators within 512 TMEM columns.
 bool mlp_tc_eligible(const MlpNet &n, int L)
 {
     const int nh = n.n_layers - 1;
-    if (nh < 1 || nh > 3 || !n.bf16_exact) return false;
-    if (L % 16 || L > 512 || n.dims[0] != L) return false;
+    if (nh < 1 || nh > 3) return false;
+    if (L % 16 || L > 4096 || n.dims[0] != L) return false;
+    const int wlim = n.bf16_exact ? kWBufBytes : 2 * kWBufBytes, per = n.bf16_exact ? 2 : 4;
     int off = 0;
     for (int l = 1; l <= nh; ++l) {
         if (n.dims[l] % 16 || n.dims[l] < 16 || n.dims[l] > 160) return false;
         off += n.dims[l];
     }
     if (off > 512) return false;
-    if (kKC * n.dims[1] * 2 > kWBufBytes) return false;
+    if (kKC * n.dims[1] * 2 > kWBufBytes / 2) return false;
     for (int l = 1; l < nh; ++l)
-        if (n.dims[l] * n.dims[l + 1] * 2 > kWBufBytes) return false;
+        if (n.dims[l] * n.dims[l + 1] * per > wlim) return false;
     // backward accumulator of layer l reuses the columns from z_(l+1) on
     int zo = 0;
     for (int l = 1; l < nh; ++l) {
@@ -507,26 +559,29 @@ bool mlp_tc_eligible(const MlpNet &n, int L)
 int mlp_tc_upload(aev_ctx *c)
 {
     const int S = c->dp.S;
-    TcAll M;
+    static TcAll M;      // 9 KB: not on the stack
     memset(&M, 0, sizeof(M));
-    for (int s = 0; s < S; ++s) {
-        const MlpNet &n = c->nets[s];
-        TcNetDev &d = M.net[s];
-        d.loaded = n.loaded;
-        if (!n.loaded || !n.tc_ok) continue;
-        d.nh = n.n_layers - 1;
-        for (int l = 0; l <= n.n_layers; ++l) d.dims[l] = n.dims[l];
-        int off = 0;
-        for (int l = 0; l < d.nh; ++l) {
-            d.wf[l] = static_cast<const __nv_bfloat16 *>(n.w_hi[l]);
-            d.wb[l] = static_cast<const __nv_bfloat16 *>(n.w_lo[l]);
-            d.bias[l] = n.bias[l];
-            d.zoff[l] = off;
-            off += n.dims[l + 1];
+    for (int m = 0; m < c->n_models; ++m)
+        for (int s = 0; s < S; ++s) {
+            const MlpNet &n = c->nets[m][s];
+            TcNetDev &d = M.net[m][s];
+            d.loaded = n.loaded;
+            if (!n.loaded || !n.tc_ok) continue;
+            d.nh = n.n_layers - 1;
+            d.need_lo = n.bf16_exact ? 0 : 1;
+            d.alpha = n.alpha;
+            for (int l = 0; l <= n.n_layers; ++l) d.dims[l] = n.dims[l];
+            int off = 0;
+            for (int l = 0; l < d.nh; ++l) {
+                d.wf[l] = static_cast<const __nv_bfloat16 *>(n.w_fwd[l]);
+                d.wb[l] = static_cast<const __nv_bfloat16 *>(n.w_bwd[l]);
+                d.bias[l] = n.bias[l];
+                d.zoff[l] = off;
+                off += n.dims[l + 1];
+            }
+            d.wlast = n.w_f32[d.nh];
+            d.blast = n.b_last;
         }
-        d.wlast = n.w_f32[d.nh];
-        d.blast = n.b_last;
-    }
     if (!c->tc_dev) AEVB_CUDA(cudaMalloc(&c->tc_dev, sizeof(TcAll)));
     AEVB_CUDA(cudaMemcpy(c->tc_dev, &M, sizeof(TcAll), cudaMemcpyHostToDevice));
     return AEV_OK;
@@ -541,29 +596,33 @@ int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *a
         AEVB_CUDA(cudaFuncSetAttribute(k_mlp_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, kTcSmem));
         c->tc_smem_optin = 1;
     }
-    dim3 grid((n_total + kTM - 1) / kTM, S);
-    launch_pdl(k_mlp_tc, grid, dim3(kTcThreads), (size_t)kTcSmem, st, static_cast<const TcAll *>(c->tc_dev), L, n_total,
-               n_atoms, (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->celu_alpha,
-               c->ws.err);
+    dim3 grid((n_total + kTM - 1) / kTM, S, c->n_models);
+    launch_pdl(k_mlp_tc, grid, dim3(kTcThreads), (size_t)kTcSmem, st, static_cast<const TcAll *>(c->tc_dev), c->n_models, L,
+               n_total, n_atoms, (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->ws.err);
     return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
 }
 
-// Host-side packing of one layer W[in][out] (row-major) into the two chunked operand layouts.
+// Host-side packing of one layer W[in][out] (row-major) into the two chunked operand layouts, each as the
+// bf16 hi parts followed by the bf16 residuals (w - hi) in the same layout.
 void mlp_tc_pack(const float *w, int K_in, int N_out, std::vector<__nv_bfloat16> &fwd, std::vector<__nv_bfloat16> &bwd,
                  bool *exact)
 {
-    fwd.assign((size_t)((K_in + 7) / 8) * N_out * 8, __float2bfloat16_rn(0.f));    // K padded to 8
-    bwd.assign((size_t)((N_out + 7) / 8) * K_in * 8, __float2bfloat16_rn(0.f));
+    const size_t nf = (size_t)((K_in + 7) / 8) * N_out * 8, nb = (size_t)((N_out + 7) / 8) * K_in * 8;   // K padded to 8
+    fwd.assign(2 * nf, __float2bfloat16_rn(0.f));
+    bwd.assign(2 * nb, __float2bfloat16_rn(0.f));
     bool ex = true;
     for (int k = 0; k < K_in; ++k)
         for (int o = 0; o < N_out; ++o) {
             const float v = w[(size_t)k * N_out + o];
             const __nv_bfloat16 b = __float2bfloat16_rn(v);
+            const __nv_bfloat16 r = __float2bfloat16_rn(v - __bfloat162float(b));
             if (__bfloat162float(b) != v) ex = false;
             // forward: B[n = o][kk = k]  ->  [kk/8][N_out][8]
-            fwd[((size_t)(k >> 3) * N_out + o) * 8 + (k & 7)] = b;
+            const size_t fi = ((size_t)(k >> 3) * N_out + o) * 8 + (k & 7);
+            fwd[fi] = b; fwd[nf + fi] = r;
             // backward: B[n = k][kk = o] ->  [kk/8][K_in][8]
-            bwd[((size_t)(o >> 3) * K_in + k) * 8 + (o & 7)] = b;
+            const size_t bi = ((size_t)(o >> 3) * K_in + k) * 8 + (o & 7);
+            bwd[bi] = b; bwd[nb + bi] = r;
         }
     *exact = ex;
 }

@@ -1,0 +1,164 @@
+"""GPU parity for the SURVEY.md 8(f) rows built in round 2: ensembles of networks,
+fp32 (non-bf16) weights and the 7-species AEV on the tensor-core MLP, the deterministic backward,
+flags and deferred errors of the host entry points.  Tolerances as in tests/test_gpu_parity.py.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from gen import ani1x_style_params, make_c5_weights, make_ensemble_weights, make_water_box, make_workload
+from gen.workloads import C5_ARCH, CELU_ALPHA
+
+from test_gpu_parity import C5_FORCE_MAX_TOL, C5_FORCE_TOL, _check_forces, _dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2310_03121_b200 as p
+    return p
+
+
+def _load_ensemble(ctx, models):
+    ctx.ani_mlp_set_ensemble(len(models))
+    for m, nets in enumerate(models):
+        for s, (ws, bs) in nets.items():
+            ctx.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
+
+
+def _energy_forces(ctx, w):
+    pos, sp, _ = _dev(w)
+    e, f = ctx.ani_energy_forces(pos, sp, w.box)
+    ctx.check_status()
+    return e.cpu().numpy(), f.cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("flags", [0, 2])
+def test_ensemble_of_eight_on_c5(pkg, flags):
+    """eight networks per species over one AEV; energy and forces are the
+    mean over the models (one AEV forward, one AEV backward).  flags = 2 runs the fp32 CUDA-core kernel."""
+    w = make_workload("C5")
+    models = make_ensemble_weights(8)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, flags=flags)
+    _load_ensemble(ctx, models)
+    e, f = _energy_forces(ctx, w)
+    we, wf, _ = oracle.energy_forces_ensemble(w.params, w.pos, w.species, w.box, models, CELU_ALPHA, use_cells=True)
+    assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    _check_forces(f, wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what=("ens8", flags))
+    # a second evaluation on the same context (the cleared mean-gradient buffer is rebuilt every call)
+    e2, f2 = _energy_forces(ctx, w)
+    assert abs(e2[0] - e[0]) <= 1e-9 * max(1.0, abs(e[0]))
+    np.testing.assert_allclose(f2, f, rtol=0, atol=1e-5 * np.abs(f).max())
+    ctx.close()
+
+
+def test_ensemble_of_identical_models_equals_one_model(pkg):
+    w = make_water_box(216, 18.64, 300, "ens-box")
+    nets = make_c5_weights()
+    c1 = pkg.Context(w.params, max_atoms=w.n_atoms)
+    for s, (ws, bs) in nets.items():
+        c1.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    e1, f1 = _energy_forces(c1, w)
+    c4 = pkg.Context(w.params, max_atoms=w.n_atoms)
+    _load_ensemble(c4, [nets] * 4)
+    e4, f4 = _energy_forces(c4, w)
+    assert abs(e4[0] - e1[0]) <= 1e-9 * max(1.0, abs(e1[0]))
+    np.testing.assert_allclose(f4, f1, rtol=0, atol=2e-5 * np.abs(f1).max())
+    c1.close(); c4.close()
+
+
+@pytest.mark.parametrize("n_models", [1, 3])
+def test_fp32_weights_stay_on_the_tensor_cores(pkg, n_models):
+    """Weights that are not bf16-representable (any trained network): hi + lo weight operands, three MMAs
+    per K step; same tolerance as the bf16 model of C5."""
+    w = make_workload("C5")
+    models = make_ensemble_weights(n_models, round_bf16=False)
+    assert any(np.any(x.view(np.uint32) & 0xFFFF) for x in models[0][0][0])
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
+    ctx.aev_set_profiling(True)
+    _load_ensemble(ctx, models)
+    e, f = _energy_forces(ctx, w)
+    we, wf, _ = oracle.energy_forces_ensemble(w.params, w.pos, w.species, w.box, models, CELU_ALPHA, use_cells=True)
+    assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    _check_forces(f, wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what=("fp32 weights on tcgen05", n_models))
+    assert ctx.mlp_kernel() == "tcgen05"
+    ctx.close()
+
+
+def test_fp32_flag_runs_the_cuda_core_kernel_within_fp32_tolerance(pkg):
+    w = make_workload("C5")
+    nets = make_c5_weights(round_bf16=False)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, flags=pkg.AEV_FLAG_MLP_FP32)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    e, f = _energy_forces(ctx, w)
+    we, wf, _ = oracle.energy_forces(w.params, w.pos, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
+    assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    _check_forces(f, wf, what="fp32 kernel")
+    assert ctx.mlp_kernel() == "fp32"
+    ctx.close()
+
+
+def test_seven_species_model_on_the_tensor_cores(pkg):
+    """ANI-2x-shaped model (seven elements): L = 1008 through k_mlp_tc (16 K-stages of layer 0,
+    8 column chunks of dE/dAEV through two alternating TMEM slots)."""
+    p7 = ani1x_style_params(num_species=7)
+    w = make_water_box(216, 18.64, 301, "s7-box")
+    rng = np.random.default_rng(70)
+    sp = rng.integers(0, 7, size=w.species.shape).astype(np.int32)
+    arch = {s: [1008] + C5_ARCH[0 if s % 2 == 0 else 3][1:] for s in range(7)}
+    nets = make_c5_weights(seed=5, arch=arch, round_bf16=(False))
+    ctx = pkg.Context(p7, max_atoms=w.n_atoms)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    e, f = ctx.ani_energy_forces(torch.from_numpy(w.pos).cuda(), torch.from_numpy(sp).cuda(), w.box)
+    ctx.check_status()
+    assert ctx.mlp_kernel() == "tcgen05"
+    we, wf, _ = oracle.energy_forces(p7, w.pos, sp, w.box, nets, CELU_ALPHA, use_cells=True)
+    assert abs(float(e[0]) - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    _check_forces(f.cpu().numpy().astype(np.float64), wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what="S=7 model")
+    ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_deterministic_flag_gives_bit_identical_forces(pkg, name):
+    """AEV_FLAG_DETERMINISTIC: neighbour contributions are accumulated in 64-bit fixed
+    point, so forces are bit-identical run to run, and still match the oracle."""
+    w = make_workload(name)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch, flags=pkg.AEV_FLAG_DETERMINISTIC)
+    pos, sp, g = _dev(w)
+    runs = []
+    for _ in range(3):
+        a = ctx.aev_forward(pos, sp, w.box).clone()
+        f = ctx.aev_backward(g).clone()
+        runs.append((a, f))
+    ctx.check_status()
+    for a, f in runs[1:]:
+        assert torch.equal(a, runs[0][0])
+        assert torch.equal(f, runs[0][1])
+    want = oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=w.box is not None)
+    _check_forces(runs[0][1].cpu().numpy(), want, what=("deterministic", name))
+    ctx.close()
+
+
+def test_host_entry_points_report_device_side_errors(pkg):
+    """a capacity overflow must not come back as AEV_OK from the synchronous host calls."""
+    w = make_workload("C1")
+    ctx = pkg.Context(w.params, max_atoms=24, max_radial_nbrs=16, max_angular_nbrs=4)
+    with pytest.raises(pkg.AevError) as e:
+        ctx.aev_forward_backward_host(w.pos, w.species, None, w.grad_aev)
+    assert e.value.code == -3
+    ctx.close()
+    # a species without a network: AEV_ERR_STATE from ani_energy_forces_host
+    ctx = pkg.Context(w.params, max_atoms=24)
+    ws, bs = make_c5_weights()[0]
+    ctx.ani_mlp_load(0, ws, bs, CELU_ALPHA)
+    with pytest.raises(pkg.AevError) as e:
+        ctx.ani_energy_forces_host(w.pos, w.species, None)
+    assert e.value.code == -4
+    ctx.close()

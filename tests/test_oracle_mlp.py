@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 
 import oracle
-from gen import ani1x_style_params, make_c1, make_c5_weights
+from gen import ani1x_style_params, make_c1, make_c5_weights, make_ensemble_weights
 from gen.workloads import C5_ARCH, CELU_ALPHA
 
 
@@ -106,3 +106,30 @@ def test_energy_forces_fd_and_net_force():
         s = int(w.species[0, i])
         tot += oracle.mlp(aev[0, i:i + 1], nets[s][0], nets[s][1], CELU_ALPHA, want_grad=False)[0][0]
     assert e[0] == pytest.approx(tot, rel=1e-13)
+
+
+def test_ensemble_of_identical_networks_is_one_network_and_fd():
+    """PAPER.md:193 (ensemble of eight models): the ensemble result is the mean over the models.
+    Pins: eight copies of one network give that network's result; the mean energy of distinct
+    networks has the ensemble forces as its negative gradient (central differences); zero net force."""
+    w = make_c1()
+    p = w.params
+    arch = {s: [384, 24, 16, 1] for s in range(4)}
+    one = make_c5_weights(seed=7, arch=arch)
+    e1, f1, _ = oracle.energy_forces(p, w.pos, w.species, None, one, CELU_ALPHA)
+    e8, f8, _ = oracle.energy_forces_ensemble(p, w.pos, w.species, None, [one] * 8, CELU_ALPHA)
+    np.testing.assert_allclose(e8, e1, rtol=1e-14)
+    np.testing.assert_allclose(f8, f1, rtol=1e-13, atol=1e-13 * np.abs(f1).max())
+    models = make_ensemble_weights(3, arch=arch, round_bf16=False)
+    e, f, _ = oracle.energy_forces_ensemble(p, w.pos, w.species, None, models, CELU_ALPHA)
+    assert abs(e[0] - e1[0]) > 1e-6          # the models really differ
+    assert np.abs(f[0].sum(axis=0)).max() < 1e-12 * np.abs(f).max()
+    rng = np.random.default_rng(11)
+    for i, a in zip(rng.integers(0, 24, 6), rng.integers(0, 3, 6)):
+        xp, xm = w.pos.copy(), w.pos.copy()
+        xp[0, i, a] = np.float32(w.pos[0, i, a] + 1e-4)
+        xm[0, i, a] = np.float32(w.pos[0, i, a] - 1e-4)
+        step = float(xp[0, i, a]) - float(xm[0, i, a])
+        ep = oracle.energy_forces_ensemble(p, xp, w.species, None, models, CELU_ALPHA)[0][0]
+        em = oracle.energy_forces_ensemble(p, xm, w.species, None, models, CELU_ALPHA)[0][0]
+        assert -(ep - em) / step == pytest.approx(f[0, i, a], rel=1e-5, abs=1e-5 * np.abs(f).max())
