@@ -52,14 +52,16 @@ struct Geom {
 
 // Device workspace owned by the context.
 struct Workspace {
-    float4 *wpos;        // [n_total] wrapped position + species bits (caller order)
     int *bin_cnt;        // [nbins_cap] member counts (zero between calls: cleared by k_nbr)
-    int *members;        // [nbins_cap*bin_cap] caller index of bin members
+    float4 *cpos;        // [nbins_cap*bin_cap] bin members: wrapped position, caller index | species << 26
+    float4 *cpos_sorted; // the same ordered by caller index inside every bin (AEV_FLAG_DETERMINISTIC, k_rank)
+    int *abin;           // [n_total] bin of every atom (AEV_FLAG_DETERMINISTIC)
     float4 *nlist;       // [n_total][cap_r] neighbour entries (dx,dy,dz, caller index j | s<<26), angular first
     int2 *ncount;        // [n_total] (nA, nB)
     int4 *hdr;           // [n_total] per atom (caller order): (nA, nB, caller index, species)
     int *noff;           // [n_total][kMaxS+1] per-species list offsets: offA | offB << 16
     int *err;            // device error flags (bitmask)
+    float4 *f4acc;       // [n_total] padded fp32 force accumulator (default mode), zero between calls
     long long *facc;     // [n_total][3] fixed-point force accumulator (AEV_FLAG_DETERMINISTIC), zero between calls
     unsigned *nbr_done;  // k_nbr CTAs that have read their bin counters (reset by the last one)
     unsigned long long *pair_count;  // export counter

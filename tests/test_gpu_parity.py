@@ -104,9 +104,9 @@ def test_aev_and_forces_match_oracle(pkg, name, cos_scale):
     ctx.close()
 
 
-def test_forward_is_run_to_run_identical_and_backward_stable(pkg):
-    """The AEV (no atomics anywhere on its path) is bit-reproducible; forces are accumulated
-    with fp32 REDs whose order may vary, so they agree to rounding only."""
+def test_run_to_run_stability_in_the_default_mode(pkg):
+    """Default mode: the order inside a cell follows k_bin's atomics and forces are accumulated with fp32
+    REDs, so two runs agree to rounding (bit-identical results: AEV_FLAG_DETERMINISTIC, tests/test_gpu_round2.py)."""
     w = make_workload("C3")
     ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
     pos, sp, g = _dev(w)
@@ -115,7 +115,7 @@ def test_forward_is_run_to_run_identical_and_backward_stable(pkg):
     a2 = ctx.aev_forward(pos, sp, w.box)
     f2 = ctx.aev_backward(g)
     ctx.check_status()
-    assert torch.equal(a1, a2)
+    assert float((a1 - a2).abs().max()) <= 1e-6 * float(a1.abs().max())
     assert float((f1 - f2).abs().max()) <= 1e-5 * float(f1.abs().max())
     ctx.close()
 
@@ -226,7 +226,7 @@ def test_host_entry_point_matches_device_entry_point(pkg):
     a1 = ctx.aev_forward(pos, sp, None).cpu().numpy()
     f1 = ctx.aev_backward(g).cpu().numpy()
     a2, f2 = ctx.aev_forward_backward_host(w.pos, w.species, None, w.grad_aev)
-    np.testing.assert_array_equal(a1, a2)
+    np.testing.assert_allclose(a1, a2, rtol=0, atol=1e-6 * np.abs(a1).max())   # order inside a cell
     np.testing.assert_allclose(f1, f2, rtol=0, atol=1e-5 * np.abs(f1).max())   # RED order
     ctx.close()
 
@@ -245,7 +245,7 @@ def test_c5_energy_and_forces(pkg):
     assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
     _check_forces(f, wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL)
     e2, f2 = ctx.ani_energy_forces_host(w.pos, w.species, w.box)
-    assert abs(e2[0] - e[0]) <= 1e-9 * max(1.0, abs(e[0]))
+    assert abs(e2[0] - e[0]) <= 1e-6 * max(1.0, abs(e[0]))      # order inside a cell, RED order
     np.testing.assert_allclose(f2, f, rtol=0, atol=1e-5 * np.abs(f).max())   # RED order
     ctx.close()
 
