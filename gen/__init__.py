@@ -13,6 +13,7 @@ from .workloads import (  # noqa: F401
     make_c1,
     make_c2,
     make_water_box,
+    make_periodic_cell,
     make_c3,
     make_c4,
     make_c5_weights,

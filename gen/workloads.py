@@ -343,6 +343,43 @@ C5_ARCH: Dict[int, List[int]] = {
 CELU_ALPHA = 0.1
 
 
+def make_periodic_cell(n_atoms: int, cell, seed: int, name: str = "cell", cos_scale: float = 1.0,
+                       min_dist: float = 1.1) -> Workload:
+    """`n_atoms` atoms of species H/C/N/O (uniform) at random positions in a small periodic cell
+    (the ML region can itself be a periodic cell of a few hundred atoms).  `cell` is three
+    edge lengths (orthorhombic) or a 3x3 matrix of lattice rows a, b, c (triclinic, reduced form).
+    Atoms are drawn one by one in fractional coordinates and rejected if closer than `min_dist` to an
+    earlier atom or within MARGIN of a cutoff (distances over the 27 nearest images, float64); a third of
+    the atoms is then moved by whole lattice vectors so that positions lie outside the cell.
+    `Workload.box` is float32 [3] or [9] (lattice rows)."""
+    p = ani1x_style_params(cos_scale)
+    rng = np.random.default_rng(seed)
+    cell = np.asarray(cell, dtype=np.float64)
+    lat = np.diag(cell) if cell.size == 3 else cell.reshape(3, 3)
+    lat = lat.astype(np.float32).astype(np.float64)
+    shifts = np.array([[i, j, k] for i in (-1, 0, 1) for j in (-1, 0, 1) for k in (-1, 0, 1)], dtype=np.float64) @ lat
+    pos = np.zeros((0, 3))
+    rcr, rca = float(p.rcr), float(p.rca)
+    tries = 0
+    while len(pos) < n_atoms:
+        tries += 1
+        if tries > 200 * n_atoms:
+            raise RuntimeError("periodic cell generator did not converge")
+        x = (rng.random(3) @ lat).astype(np.float32).astype(np.float64)
+        if len(pos):
+            d = (pos[:, None, :] - x[None, None, :]) + shifts[None, :, :]
+            r = np.sqrt((d * d).sum(axis=2)).min(axis=1)
+            if r.min() < min_dist or (np.abs(r - rcr) < 10 * MARGIN).any() or (np.abs(r - rca) < 10 * MARGIN).any():
+                continue
+        pos = np.vstack([pos, x])
+    move = rng.random(n_atoms) < 0.33
+    pos = pos + np.where(move[:, None], rng.integers(-2, 3, size=(n_atoms, 3)).astype(np.float64) @ lat, 0.0)
+    species = rng.integers(0, 4, size=n_atoms).astype(np.int32)
+    box = (cell if cell.size == 3 else lat.reshape(9)).astype(np.float32)
+    return Workload(name, pos.astype(np.float32)[None], species[None], box,
+                    _grad_aev((1, n_atoms, p.aev_length), seed), p)
+
+
 def _round_to_bf16(x: np.ndarray) -> np.ndarray:
     """Round float32 to the nearest bf16-representable float32 (ties to even)."""
     u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)

@@ -41,8 +41,11 @@
  * n_shf_r == 16, n_shf_a == 4, n_shf_z == 8 (the shift counts of BASELINE.json:configs[0],
  * "ANI-1x-style"; the lane mappings of the kernels are built on 16 / 4 x 8 = 32), zeta a power
  * of two in [1,64], 0 < rca <= rcr, 0 < cos_scale <= 1; periodic boxes are orthorhombic (three
- * edge lengths) or, with AEV_FLAG_TRICLINIC, reduced triclinic (three lattice vectors), every
- * perpendicular width >= 2*rcr.
+ * edge lengths, each >= 2*rcr) or, with AEV_FLAG_TRICLINIC, reduced triclinic (three lattice
+ * vectors, ax, by, cz >= 2*rcr).  Orthorhombic boxes with at least 3 cells of edge >= rcr along every
+ * axis use the cell list; smaller ones and every triclinic box are searched as one cell with the
+ * minimum image taken per pair (O(n^2) candidate tests: meant for ML regions of a few hundred atoms,
+ * such as the 528-atom periodic cell of PAPER.md:223).
  */
 #ifndef AEV_B200_H
 #define AEV_B200_H
@@ -56,7 +59,7 @@ extern "C" {
 enum {
     AEV_OK = 0,
     AEV_ERR_INVALID_ARG = -1,   /* null pointer, bad shape, n > max_atoms, ...                 */
-    AEV_ERR_BOX_TOO_SMALL = -2, /* a periodic edge < 2*rcr (no unique minimum image) or < 3 cells */
+    AEV_ERR_BOX_TOO_SMALL = -2, /* a periodic edge (triclinic: ax, by or cz) < 2*rcr: no unique minimum image  */
     AEV_ERR_CAPACITY = -3,      /* a per-atom neighbour capacity or a cell capacity overflowed
                                    on the device; results of that call are incomplete          */
     AEV_ERR_STATE = -4,         /* aev_backward without a preceding aev_forward, MLP not loaded */
@@ -118,6 +121,7 @@ int aev_length(const aev_ctx *c);
  *   species  device i32 [batch][n_atoms]; id < 0 = padding atom (belongs to no pair)
  *   box      HOST f32[3] orthorhombic edge lengths (shared by the batch), or NULL =
  *            non-periodic all-pairs within each system.  Positions may lie outside [0,L).
+ *            On a context created with AEV_FLAG_TRICLINIC: HOST f32[9], lattice rows a, b, c.
  * Builds, inside the context, per-atom neighbour lists (angular-set neighbours first) that
  * aev_export_pairs can read back.  Asynchronous.
  */
@@ -191,6 +195,24 @@ int ani_mlp_load_model(aev_ctx *c, int32_t model, int32_t species, int32_t n_lay
 int ani_energy_forces(aev_ctx *c, const float *pos, const int32_t *species, const float *box,
                       int32_t n_atoms, int32_t batch, double *energy_out, float *forces_out,
                       void *stream);
+
+/*
+ * The ML region of a mixed ML/MM system (createMixedSystem(topology, mm_system, ml_atoms);
+ * 53 ML atoms of 134,099): energy and forces of the n_ml atoms listed in ml_index, evaluated
+ * as one non-batched system of their own (positions gathered from the full array by a kernel), and the
+ * ML forces ADDED onto forces_all at those atoms (the MM forces already there are kept; every other
+ * entry is left untouched).
+ *   pos_all     device f32 [n_all][3]     positions of the whole system
+ *   ml_index    device i32 [n_ml]         distinct indices into pos_all / forces_all
+ *   species_ml  device i32 [n_ml]         species of the ML atoms, in ml_index order
+ *   box         HOST, as for aev_forward (NULL = the usual gas-phase ML region)
+ *   energy_out  device f64 [1]
+ *   forces_all  device f32 [n_all][3]     forces_all[ml_index[k]] += F_ml[k]
+ * n_ml <= max_atoms.  Asynchronous.
+ */
+int ani_energy_forces_subset(aev_ctx *c, const float *pos_all, const int32_t *ml_index,
+                             const int32_t *species_ml, const float *box, int32_t n_ml,
+                             double *energy_out, float *forces_all, void *stream);
 
 /*
  * Host-buffer convenience entry points (the "end to end" calls bench.py times): every

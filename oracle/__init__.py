@@ -56,6 +56,8 @@ def lib():
         L.oracle_aev_backward.restype = C.c_int
         L.oracle_aev_backward.argtypes = [C.POINTER(_Params), f32p, i32p, f32p, C.c_int32, C.c_int32,
                                           C.c_int, f32p, f64p]
+        L.oracle_set_lattice.restype = C.c_int
+        L.oracle_set_lattice.argtypes = [f64p]
         L.oracle_mlp.restype = C.c_int
         L.oracle_mlp.argtypes = [C.c_int32, f64p, C.c_int32, i32p, C.POINTER(f64p), C.POINTER(f64p),
                                  C.c_double, f64p, f64p]
@@ -98,6 +100,26 @@ class _P:
                          len(self.shf_a), _ptr(self.shf_a, C.c_double),
                          len(self.shf_z), _ptr(self.shf_z, C.c_double),
                          f(p.cos_scale))
+
+
+class lattice:
+    """Context manager: inside it every periodic displacement is the minimum image of the triclinic cell
+    with rows a, b, c (`box` arguments are then ignored and the cell list is not available):
+
+        with oracle.lattice(lat): aev = oracle.aev_forward(p, pos, species, None)
+    """
+
+    def __init__(self, lat):
+        self.lat = np.ascontiguousarray(np.asarray(lat, dtype=np.float32).astype(np.float64).reshape(9))
+
+    def __enter__(self):
+        if lib().oracle_set_lattice(_ptr(self.lat, C.c_double)) != 0:
+            raise ValueError("singular lattice")
+        return self
+
+    def __exit__(self, *exc):
+        lib().oracle_set_lattice(None)
+        return False
 
 
 def aev_length(p) -> int:

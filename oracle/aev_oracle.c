@@ -78,8 +78,49 @@ void oracle_set_threads(int n)
 }
 
 /* ------------------------------------------------------------------ step 1: pairs */
+/* Triclinic cell (PAPER.md:223 names periodic ML cells): when a lattice is
+ * set, `box` arguments are ignored and the displacement is the SHORTEST of x_j - x_i - (na a + nb b + nc c)
+ * over the image shifts na, nb, nc in {-2..2} around the fractional-coordinate rounding -- the definition
+ * of the minimum image written as a search (125 candidates), not the sequential rint the CUDA path uses.
+ * Valid for lattices whose perpendicular widths exceed 2 R_c.  Set / cleared from one thread before a call. */
+static int g_tri = 0;
+static double g_lat[9], g_inv[9];   /* rows a, b, c; inverse such that frac = v * g_inv (row vector) */
+
+int oracle_set_lattice(const double *lat)
+{
+    if (!lat) { g_tri = 0; return 0; }
+    const double *a = lat, *b = lat + 3, *c = lat + 6;
+    double det = a[0] * (b[1] * c[2] - b[2] * c[1]) - a[1] * (b[0] * c[2] - b[2] * c[0])
+               + a[2] * (b[0] * c[1] - b[1] * c[0]);
+    if (!(fabs(det) > 0.0)) return -1;
+    memcpy(g_lat, lat, sizeof(g_lat));
+    /* inverse of the matrix with rows a, b, c (cofactors / det) */
+    g_inv[0] = (b[1] * c[2] - b[2] * c[1]) / det; g_inv[1] = (a[2] * c[1] - a[1] * c[2]) / det; g_inv[2] = (a[1] * b[2] - a[2] * b[1]) / det;
+    g_inv[3] = (b[2] * c[0] - b[0] * c[2]) / det; g_inv[4] = (a[0] * c[2] - a[2] * c[0]) / det; g_inv[5] = (a[2] * b[0] - a[0] * b[2]) / det;
+    g_inv[6] = (b[0] * c[1] - b[1] * c[0]) / det; g_inv[7] = (a[1] * c[0] - a[0] * c[1]) / det; g_inv[8] = (a[0] * b[1] - a[1] * b[0]) / det;
+    g_tri = 1;
+    return 0;
+}
+
 static inline void displacement(const float *pos, const float *box, int64_t i, int64_t j, double d[3])
 {
+    if (g_tri) {
+        double v[3], f[3];
+        for (int a = 0; a < 3; ++a) v[a] = (double)pos[3 * j + a] - (double)pos[3 * i + a];
+        /* fractional coordinates of v, rounded: brings v next to the origin cell */
+        for (int k = 0; k < 3; ++k) f[k] = rint(v[0] * g_inv[k] + v[1] * g_inv[3 + k] + v[2] * g_inv[6 + k]);
+        for (int a = 0; a < 3; ++a) v[a] -= f[0] * g_lat[a] + f[1] * g_lat[3 + a] + f[2] * g_lat[6 + a];
+        double best = -1.0;
+        for (int na = -2; na <= 2; ++na)
+            for (int nb = -2; nb <= 2; ++nb)
+                for (int nc = -2; nc <= 2; ++nc) {
+                    double w[3];
+                    for (int a = 0; a < 3; ++a) w[a] = v[a] - (na * g_lat[a] + nb * g_lat[3 + a] + nc * g_lat[6 + a]);
+                    double r2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2];
+                    if (best < 0.0 || r2 < best) { best = r2; d[0] = w[0]; d[1] = w[1]; d[2] = w[2]; }
+                }
+        return;
+    }
     for (int a = 0; a < 3; ++a) {
         double v = (double)pos[3 * j + a] - (double)pos[3 * i + a];
         if (box) {

@@ -28,7 +28,7 @@ ERRORS = {
 
 EXPORTS = [
     "aev_create", "aev_destroy", "aev_length", "aev_neighbors", "aev_forward", "aev_backward",
-    "ani_mlp_load", "ani_mlp_set_ensemble", "ani_mlp_load_model", "ani_mlp_kernel", "ani_energy_forces", "aev_forward_backward_host", "ani_energy_forces_host",
+    "ani_mlp_load", "ani_mlp_set_ensemble", "ani_mlp_load_model", "ani_mlp_kernel", "ani_energy_forces", "ani_energy_forces_subset", "aev_forward_backward_host", "ani_energy_forces_host",
     "aev_export_pairs", "aev_export_counts", "aev_set_profiling", "aev_get_profile", "aev_status", "aev_launch_count", "aev_probe_fp32_tflops",
     "aev_error_string",
 ]
@@ -102,6 +102,8 @@ def lib():
         L.ani_mlp_kernel.argtypes = [vp]
         L.ani_energy_forces.restype = C.c_int
         L.ani_energy_forces.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, vp, f32p, vp]
+        L.ani_energy_forces_subset.restype = C.c_int
+        L.ani_energy_forces_subset.argtypes = [vp, f32p, i32p, i32p, C.POINTER(C.c_float), i32, vp, f32p, vp]
         L.aev_forward_backward_host.restype = C.c_int
         L.aev_forward_backward_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), i32, i32, vp, vp, vp]
         L.ani_energy_forces_host.restype = C.c_int
@@ -134,7 +136,9 @@ def _check(rc: int, where: str) -> None:
 def _box(box):
     if box is None:
         return None, None
-    arr = np.ascontiguousarray(np.asarray(box, dtype=np.float32).reshape(3))
+    arr = np.ascontiguousarray(np.asarray(box, dtype=np.float32).reshape(-1))      # 3 edges, or 9 with AEV_FLAG_TRICLINIC
+    if arr.size not in (3, 9):
+        raise ValueError("box must have 3 (orthorhombic) or 9 (triclinic lattice rows) entries")
     return arr, arr.ctypes.data_as(C.POINTER(C.c_float))
 
 
@@ -261,6 +265,22 @@ class Context:
                                        _dev_ptr(forces_out, torch.float32, "forces_out"),
                                        _stream(stream)), "ani_energy_forces")
         return energy_out, forces_out
+
+    def ani_energy_forces_subset(self, pos_all, ml_index, species_ml, forces_all, box=None, energy_out=None,
+                                 stream=None):
+        """ML region of a mixed system: forces_all[ml_index] += F_ml (in place); returns the energy tensor."""
+        import torch
+        if energy_out is None:
+            energy_out = torch.empty((1,), dtype=torch.float64, device=pos_all.device)
+        keep, bp = _box(box)
+        _check(lib().ani_energy_forces_subset(self._h, _dev_ptr(pos_all, torch.float32, "pos_all"),
+                                              _dev_ptr(ml_index, torch.int32, "ml_index"),
+                                              _dev_ptr(species_ml, torch.int32, "species_ml"), bp,
+                                              int(ml_index.numel()),
+                                              _dev_ptr(energy_out, torch.float64, "energy_out"),
+                                              _dev_ptr(forces_all, torch.float32, "forces_all"),
+                                              _stream(stream)), "ani_energy_forces_subset")
+        return energy_out
 
     # -- host-buffer calls (numpy in / out; synchronous)
     def aev_forward_backward_host(self, pos: np.ndarray, species: np.ndarray, box, grad_aev: Optional[np.ndarray],

@@ -41,7 +41,11 @@ struct DevParams {
 // Geometry of one call (filled on the host per call, passed by value).
 struct Geom {
     int n_atoms, batch, n_total;
-    int periodic;
+    int periodic;                // 1: cell grid with a 27-cell stencil and image shifts per stencil cell
+    int mi;                      // 1: one cell per system, all pairs, minimum image taken in the distance test (boxes
+                                 //    with fewer than 3 cells along an edge, and every triclinic box)
+    float lat[9];                // mi: lattice rows a = (ax,0,0), b = (bx,by,0), c = (cx,cy,cz) (orthorhombic: diagonal)
+    float inv_diag[3];           // mi: 1/ax, 1/by, 1/cz
     int ncx, ncy, ncz, ncell;    // cells per system (non-periodic: 1,1,1,1)
     int nbins;                   // batch*ncell*S
     int bin_cap;                 // capacity of one (cell,species) member list
@@ -112,6 +116,7 @@ struct aev_ctx {
     int *sp_count;               // [S]
     void *tc_dev;                // device copy of the tensor-core network table (ani_mlp_tc.cu)
     void *f32_dev;               // device copy of the fp32 network table (ani_mlp.cu)
+    float *sub_buf;              // [max_atoms][3] gathered positions | [max_atoms][3] forces (ani_energy_forces_subset)
     // host staging (pinned) + device staging for the *_host entry points
     int profiling;
     void *prof;                  // std::vector<ProfRec>* (aev_kernels.cu)

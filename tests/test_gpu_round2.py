@@ -162,3 +162,91 @@ def test_host_entry_points_report_device_side_errors(pkg):
         ctx.ani_energy_forces_host(w.pos, w.species, None)
     assert e.value.code == -4
     ctx.close()
+
+
+# --------------------------------------------------------------------------- small and triclinic cells (8(f) rank 3)
+def _check_cell(pkg, w, flags=0, lattice=None):
+    from test_gpu_parity import AEV_TOL
+    import contextlib
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, flags=flags)
+    pos, sp, g = _dev(w)
+    ctx.aev_neighbors(pos, sp, w.box)
+    ctx.check_status()
+    scope = oracle.lattice(lattice) if lattice is not None else contextlib.nullcontext()
+    obox = None if lattice is not None else w.box
+    with scope:
+        for which, rc in ((0, w.params.rcr), (1, w.params.rca)):
+            got = ctx.aev_export_pairs(which, cap=w.n_atoms * 80)
+            want = oracle.pairs(w.pos[0], w.species[0], obox, float(rc), "brute").astype(np.int32)
+            np.testing.assert_array_equal(got, want)
+        want_a = oracle.aev_forward(w.params, w.pos, w.species, obox)
+        want_f = oracle.aev_backward(w.params, w.pos, w.species, obox, w.grad_aev)
+    aev = ctx.aev_forward(pos, sp, w.box)
+    f = ctx.aev_backward(g)
+    ctx.check_status()
+    assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+    _check_forces(f.cpu().numpy(), want_f, what=(w.name, flags))
+    ctx.close()
+
+
+@pytest.mark.parametrize("cell", [(12.0, 13.0, 14.5), (11.0, 24.0, 17.0)])
+def test_orthorhombic_boxes_with_fewer_than_three_cells_per_edge(pkg, cell):
+    """PAPER.md:223 (a 528-atom periodic ML cell): edges between 2*R_cr and 3 cells (10.4 .. 15.6 A) are searched as
+    one cell with the minimum image per pair; (11, 24, 17) has one short and two long edges."""
+    from gen import make_periodic_cell
+    n = int(0.1 * cell[0] * cell[1] * cell[2])
+    _check_cell(pkg, make_periodic_cell(n, cell, 45, name="small-box"))
+
+
+@pytest.mark.parametrize("det", [0, 1])
+def test_triclinic_cell(pkg, det):
+    from gen import make_periodic_cell
+    lat = [[14.0, 0.0, 0.0], [3.0, 13.0, 0.0], [-2.0, 4.0, 12.5]]
+    w = make_periodic_cell(240, lat, 46, name="triclinic")
+    _check_cell(pkg, w, flags=pkg.AEV_FLAG_TRICLINIC | det, lattice=w.box)
+
+
+def test_triclinic_argument_checks(pkg):
+    p = ani1x_style_params()
+    ctx = pkg.Context(p, max_atoms=8, flags=pkg.AEV_FLAG_TRICLINIC)
+    pos = torch.rand((1, 8, 3), device="cuda") * 5
+    sp = torch.zeros((1, 8), dtype=torch.int32, device="cuda")
+    with pytest.raises(pkg.AevError) as e:      # not reduced: |bx| > ax/2
+        ctx.aev_forward(pos, sp, np.array([14, 0, 0, 9, 13, 0, 0, 0, 12], dtype=np.float32))
+    assert e.value.code == -1
+    with pytest.raises(pkg.AevError) as e:      # cz < 2 R_cr
+        ctx.aev_forward(pos, sp, np.array([14, 0, 0, 3, 13, 0, 0, 0, 9], dtype=np.float32))
+    assert e.value.code == -2
+    ctx.close()
+
+
+# --------------------------------------------------------------------------- ml_atoms of a mixed system (8(f) rank 2)
+def test_ml_subset_gathers_positions_and_adds_forces(pkg):
+    """a 60-atom ML region inside a 4,500-atom system; the ML forces are added onto the
+    (MM) forces already in the array, every other entry stays bit-identical."""
+    big = make_workload("C3")
+    lig = make_workload("C2")
+    rng = np.random.default_rng(9)
+    n_all, n_ml = big.n_atoms, lig.n_atoms
+    idx = np.sort(rng.choice(n_all, size=n_ml, replace=False)).astype(np.int32)
+    idx = rng.permutation(idx).astype(np.int32)
+    pos_all = big.pos[0].copy()
+    pos_all[idx] = lig.pos[0]                       # conformer 0 of the ligand sits at the ML indices
+    sp_ml = lig.species[0].copy()
+    f_mm = rng.standard_normal((n_all, 3)).astype(np.float32)
+    nets = make_c5_weights(seed=3, arch={s: [384, 96, 64, 1] for s in range(4)})
+    ctx = pkg.Context(lig.params, max_atoms=n_ml)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    f_all = torch.from_numpy(f_mm.copy()).cuda()
+    e = ctx.ani_energy_forces_subset(torch.from_numpy(pos_all).cuda(), torch.from_numpy(idx).cuda(),
+                                     torch.from_numpy(sp_ml).cuda(), f_all)
+    ctx.check_status()
+    we, wf, _ = oracle.energy_forces(lig.params, lig.pos[:1], lig.species[:1], None, nets, CELU_ALPHA)
+    got = f_all.cpu().numpy()
+    assert abs(float(e[0]) - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    rest = np.ones(n_all, dtype=bool)
+    rest[idx] = False
+    np.testing.assert_array_equal(got[rest], f_mm[rest])
+    _check_forces((got[idx].astype(np.float64) - f_mm[idx])[None], wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what="ml subset")
+    ctx.close()

@@ -443,3 +443,95 @@ def test_collinear_triplet_literal_angle_cone_point():
     a2 = oracle.aev_forward(ani1x_style_params(1.0 - 1e-7), pos, sp, None)
     # theta moves by sqrt(2e-7) = 4.5e-4 rad; zeta = 32 amplifies: a continuity check, not an identity
     np.testing.assert_allclose(a1, a2, rtol=0, atol=1e-2 * np.abs(a1).max())
+
+
+# --------------------------------------------------------------------------- triclinic cells
+TRI_LAT = np.array([[14.0, 0.0, 0.0], [3.0, 13.0, 0.0], [-2.0, 4.0, 12.5]])
+
+
+def test_lattice_mode_with_a_diagonal_lattice_is_the_orthorhombic_minimum_image():
+    """The triclinic image search (oracle.lattice) reduces to the already pinned L*rint(d/L) routine when the
+    lattice is diagonal: same pair sets, AEV and forces."""
+    from gen import make_periodic_cell
+    w = make_periodic_cell(160, [12.0, 13.0, 14.5], 42)
+    g = w.grad_aev
+    a1 = oracle.aev_forward(w.params, w.pos, w.species, w.box)
+    f1 = oracle.aev_backward(w.params, w.pos, w.species, w.box, g)
+    p1 = oracle.pairs(w.pos[0], w.species[0], w.box, float(w.params.rcr))
+    with oracle.lattice(np.diag(w.box)):
+        a2 = oracle.aev_forward(w.params, w.pos, w.species, None)
+        f2 = oracle.aev_backward(w.params, w.pos, w.species, None, g)
+        p2 = oracle.pairs(w.pos[0], w.species[0], None, float(w.params.rcr))
+    np.testing.assert_array_equal(p1, p2)
+    np.testing.assert_allclose(a2, a1, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(f2, f1, rtol=0, atol=1e-11 * np.abs(f1).max())
+
+
+def test_triclinic_cell_equals_its_explicit_replication():
+    """A periodic triclinic cell is, by definition, the infinite lattice of its copies: the AEV rows and forces of
+    the cell's atoms must equal those of the same atoms inside a NON-periodic cluster of 5x5x5 explicit copies
+    (every neighbour within R_cr of a central-copy atom lies in that cluster).  This checks the image search
+    against plain open-boundary arithmetic that does not use it."""
+    from gen import make_periodic_cell
+    w = make_periodic_cell(40, TRI_LAT, 43, min_dist=1.3)
+    n = w.n_atoms
+    lat = w.box.reshape(3, 3).astype(np.float64)
+    g = w.grad_aev
+    with oracle.lattice(w.box):
+        a_p = oracle.aev_forward(w.params, w.pos, w.species, None)
+        f_p = oracle.aev_backward(w.params, w.pos, w.species, None, g)
+        pr = oracle.pairs(w.pos[0], w.species[0], None, float(w.params.rcr))
+    # the cluster: wrap every atom into the cell first (copies of an atom far outside would leave the 5x5x5 block)
+    frac = w.pos[0].astype(np.float64) @ np.linalg.inv(lat)
+    base = (frac - np.floor(frac)) @ lat
+    shifts = [np.array([i, j, k], dtype=np.float64) @ lat for i in range(-2, 3) for j in range(-2, 3) for k in range(-2, 3)]
+    centre = len(shifts) // 2
+    assert np.all(shifts[centre] == 0.0)
+    big = np.concatenate([base + s for s in shifts]).astype(np.float64)
+    big_sp = np.tile(w.species[0], len(shifts))
+    # float32 inputs: use the replicated float64 positions rounded once, and the same rounded base inside the cell
+    big32 = big.astype(np.float32)
+    lo, hi = centre * n, (centre + 1) * n
+    with oracle.lattice(w.box):
+        a_p = oracle.aev_forward(w.params, big32[lo:hi][None], w.species, None)
+        pr = oracle.pairs(big32[lo:hi], w.species[0], None, float(w.params.rcr))
+    a_c = oracle.aev_forward(w.params, big32[None], big_sp[None], None)[:, lo:hi]
+    # float32 rounding of the replicas' coordinates moves distances by ~1e-6 A: compare at that level
+    np.testing.assert_allclose(a_p, a_c, rtol=0, atol=2e-5 * np.abs(a_c).max())
+    # pair set: periodic pairs (i<j) <-> cluster pairs with one end in the central copy, folded back to (i, j mod n)
+    pc = oracle.pairs(big32, big_sp, None, float(w.params.rcr))
+    inc = (pc[:, 0] >= lo) & (pc[:, 0] < hi) | (pc[:, 1] >= lo) & (pc[:, 1] < hi)
+    fold = np.sort(np.stack([pc[inc, 0] % n, pc[inc, 1] % n], axis=1), axis=1)
+    fold = np.unique(fold[fold[:, 0] != fold[:, 1]], axis=0)
+    np.testing.assert_array_equal(fold, pr)
+    # forces: upstream gradient only on the central copy's rows; the force on a periodic atom is the sum over its copies
+    gbig = np.zeros((1, len(big32), g.shape[2]), dtype=np.float32)
+    gbig[0, lo:hi] = g[0]
+    f_c = oracle.aev_backward(w.params, big32[None], big_sp[None], None, gbig)[0].reshape(len(shifts), n, 3).sum(axis=0)
+    with oracle.lattice(w.box):
+        f_p = oracle.aev_backward(w.params, big32[lo:hi][None], w.species, None, g)[0]
+    np.testing.assert_allclose(f_p, f_c, rtol=0, atol=2e-4 * np.abs(f_c).max())
+
+
+def test_triclinic_lattice_translation_invariance_and_finite_differences():
+    from gen import make_periodic_cell
+    w = make_periodic_cell(60, TRI_LAT, 44)
+    lat = w.box.reshape(3, 3).astype(np.float64)
+    g = w.grad_aev
+    rng = np.random.default_rng(3)
+    with oracle.lattice(w.box):
+        a0 = oracle.aev_forward(w.params, w.pos, w.species, None)
+        f0 = oracle.aev_backward(w.params, w.pos, w.species, None, g)
+        moved = w.pos.copy()
+        moved[0] += (rng.integers(-1, 2, size=(w.n_atoms, 3)).astype(np.float64) @ lat).astype(np.float32)
+        a1 = oracle.aev_forward(w.params, moved, w.species, None)
+        np.testing.assert_allclose(a1, a0, rtol=0, atol=3e-5 * np.abs(a0).max())     # float32 coordinates of the moved atoms
+        assert np.abs(f0[0].sum(axis=0)).max() < 1e-10 * np.abs(f0).max() * w.n_atoms
+        for i, c in zip(rng.integers(0, w.n_atoms, 5), rng.integers(0, 3, 5)):
+            xp, xm = w.pos.copy(), w.pos.copy()
+            xp[0, i, c] = np.float32(w.pos[0, i, c] + 1e-4)
+            xm[0, i, c] = np.float32(w.pos[0, i, c] - 1e-4)
+            step = float(xp[0, i, c]) - float(xm[0, i, c])
+            ep = (oracle.aev_forward(w.params, xp, w.species, None) * g).sum()
+            em = (oracle.aev_forward(w.params, xm, w.species, None) * g).sum()
+            assert -(ep - em) / step == pytest.approx(f0[0, i, c], rel=2e-5, abs=2e-5 * np.abs(f0).max())
