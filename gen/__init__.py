@@ -19,5 +19,6 @@ from .workloads import (  # noqa: F401
     make_c5_weights,
     make_ensemble_weights,
     make_workload,
+    random_walk,
     Workload,
 )

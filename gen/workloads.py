@@ -380,6 +380,33 @@ def make_periodic_cell(n_atoms: int, cell, seed: int, name: str = "cell", cos_sc
                     _grad_aev((1, n_atoms, p.aev_length), seed), p)
 
 
+def random_walk(w: Workload, n_steps: int, sigma: float, seed: int) -> List[np.ndarray]:
+    """MD-like trajectory for the neighbour-list reuse tests (10,000 consecutive steps): every step adds
+    N(0, sigma) to every coordinate; atoms that end up within MARGIN of a cutoff (or nearly collinear) get a new
+    draw, so that every frame keeps the generators' guarantee.  Returns n_steps float32 arrays shaped like w.pos."""
+    rng = np.random.default_rng(seed)
+    frames = []
+    cur = w.pos.astype(np.float64)
+    p = w.params
+    for _ in range(n_steps):
+        step = rng.normal(0.0, sigma, size=cur.shape)
+        for _try in range(50):
+            new = (cur + step).astype(np.float32)
+            bad_any = False
+            for b in range(new.shape[0]):
+                bad = _bad_atoms(new[b], w.box, float(p.rcr), float(p.rca))
+                if len(bad):
+                    bad_any = True
+                    step[b, bad] = rng.normal(0.0, sigma, size=(len(bad), 3))
+            if not bad_any:
+                break
+        else:
+            raise RuntimeError("random walk repair did not converge")
+        frames.append(new)
+        cur = new.astype(np.float64)
+    return frames
+
+
 def _round_to_bf16(x: np.ndarray) -> np.ndarray:
     """Round float32 to the nearest bf16-representable float32 (ties to even)."""
     u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)

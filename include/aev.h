@@ -254,6 +254,9 @@ int aev_get_profile(aev_ctx *c, double *ms_out, int64_t *n_out);
 /* Syncs the context's last stream and returns AEV_OK or the deferred device-side error
  * (AEV_ERR_CAPACITY, AEV_ERR_STATE) raised by any call since the last aev_status. */
 int aev_status(aev_ctx *c);
+/* Verlet-skin mode (aev_params.skin > 0): how many times the neighbour lists have been rebuilt so far (the
+ * other calls reused them).  Syncs.  AEV_ERR_STATE on a context without a skin (every call builds). */
+int aev_neighbor_builds(aev_ctx *c, int64_t *builds_out);
 /* Number of kernels the library has launched on this context so far (bench bookkeeping). */
 int64_t aev_launch_count(const aev_ctx *c);
 /* Independent-FMA microbenchmark: measured FP32 FMA throughput of `device` in TFLOP/s

@@ -29,7 +29,7 @@ ERRORS = {
 EXPORTS = [
     "aev_create", "aev_destroy", "aev_length", "aev_neighbors", "aev_forward", "aev_backward",
     "ani_mlp_load", "ani_mlp_set_ensemble", "ani_mlp_load_model", "ani_mlp_kernel", "ani_energy_forces", "ani_energy_forces_subset", "aev_forward_backward_host", "ani_energy_forces_host",
-    "aev_export_pairs", "aev_export_counts", "aev_set_profiling", "aev_get_profile", "aev_status", "aev_launch_count", "aev_probe_fp32_tflops",
+    "aev_export_pairs", "aev_export_counts", "aev_set_profiling", "aev_get_profile", "aev_status", "aev_launch_count", "aev_neighbor_builds", "aev_probe_fp32_tflops",
     "aev_error_string",
 ]
 
@@ -118,6 +118,8 @@ def lib():
         L.aev_get_profile.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
         L.aev_status.restype = C.c_int
         L.aev_status.argtypes = [vp]
+        L.aev_neighbor_builds.restype = C.c_int
+        L.aev_neighbor_builds.argtypes = [vp, C.POINTER(i64)]
         L.aev_launch_count.restype = i64
         L.aev_launch_count.argtypes = [vp]
         L.aev_probe_fp32_tflops.restype = C.c_int
@@ -352,6 +354,11 @@ class Context:
 
     def check_status(self):
         _check(self.aev_status(), "aev_status")
+
+    def neighbor_builds(self) -> int:
+        out = C.c_int64(0)
+        _check(lib().aev_neighbor_builds(self._h, C.byref(out)), "aev_neighbor_builds")
+        return int(out.value)
 
     def launch_count(self) -> int:
         return int(lib().aev_launch_count(self._h))

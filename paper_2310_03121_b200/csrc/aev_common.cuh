@@ -65,6 +65,16 @@ struct Workspace {
     int4 *hdr;           // [n_total] per atom (caller order): (nA, nB, caller index, species)
     int *noff;           // [n_total][kMaxS+1] per-species list offsets: offA | offB << 16
     int *err;            // device error flags (bitmask)
+    // Verlet-skin reuse (aev_params.skin > 0): lists built with rcr+skin / rca+skin, filtered every call by k_refresh
+    float4 *vlist;       // [n_total][vcap_r]
+    int2 *vcount;        // [n_total]
+    int4 *vhdr;          // [n_total]
+    int *vnoff;          // [n_total][kMaxS+1]
+    float *pos_ref;      // [n_total][3] positions at the last build
+    float4 *pos4;        // [n_total] this call's positions, padded (k_disp writes, k_refresh gathers)
+    int *need;           // 1: this call rebuilds the Verlet lists (set by k_disp, cleared by k_refresh); NULL without skin
+    int *valid;          // 1: the Verlet lists match the current shapes (set by k_nbr, cleared by the host)
+    unsigned long long *builds;   // Verlet-list builds so far
     float4 *f4acc;       // [n_total] padded fp32 force accumulator (default mode), zero between calls
     long long *facc;     // [n_total][3] fixed-point force accumulator (AEV_FLAG_DETERMINISTIC), zero between calls
     unsigned *nbr_done;  // k_nbr CTAs that have read their bin counters (reset by the last one)
@@ -101,6 +111,9 @@ struct aev_ctx {
     cudaStream_t last_stream;
     size_t cap_total;            // atoms the workspace is sized for
     size_t nbins_cap, members_cap;
+    int vcap_r, vcap_a;          // per-atom capacities of the Verlet lists
+    aevb::Geom vgeom;            // geometry of the last call in skin mode (a change invalidates the Verlet lists)
+    int vgeom_set;
     int fwd_smem_optin;          // bytes of dynamic smem the forward kernels were opted into (per device => per ctx)
     size_t bwd_smem_optin, mlp_smem_optin;
     int tc_smem_optin;

@@ -250,3 +250,93 @@ def test_ml_subset_gathers_positions_and_adds_forces(pkg):
     np.testing.assert_array_equal(got[rest], f_mm[rest])
     _check_forces((got[idx].astype(np.float64) - f_mm[idx])[None], wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what="ml subset")
     ctx.close()
+
+
+# --------------------------------------------------------------------------- Verlet-skin reuse (8(f) rank 2)
+@pytest.mark.parametrize("kind", ["water-box", "gas-batch", "small-cell"])
+def test_verlet_skin_random_walk_matches_a_rebuild_every_step(pkg, kind):
+    """PAPER.md:199 (10,000 consecutive MD steps): with aev_params.skin the lists are rebuilt only when an atom has
+    moved more than skin/2; the exact cutoffs are applied when the lists are read, so every frame of a 20-step
+    random walk gives the pair sets (bit-exact), AEV and forces of a context that rebuilds every call, and of the
+    oracle.  Half-way the whole system is shifted by box vectors (a wrap is not a displacement)."""
+    from gen import make_periodic_cell, random_walk
+    from test_gpu_parity import AEV_TOL
+    if kind == "water-box":
+        w = make_water_box(216, 18.64, 310, "skin-box")
+    elif kind == "gas-batch":
+        w0 = make_workload("C2")
+        w = type(w0)("skin-gas", w0.pos[:8].copy(), w0.species[:8].copy(), None, w0.grad_aev[:8].copy(), w0.params)
+    else:
+        w = make_periodic_cell(180, (13.0, 13.5, 14.0), 47, name="skin-cell")
+    frames = random_walk(w, 20, 0.04, 5)
+    skin = 0.6
+    cs = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch, skin=skin)
+    cr = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch)
+    sp = torch.from_numpy(w.species).cuda()
+    g = torch.from_numpy(w.grad_aev).cuda()
+    for t, fr in enumerate(frames):
+        fr = fr.copy()
+        if w.box is not None and t >= 10:
+            fr[:, ::3] += (np.asarray(w.box[:3]) * np.array([1, -1, 1])).astype(np.float32)
+        pos = torch.from_numpy(fr).cuda()
+        a_s = cs.aev_forward(pos, sp, w.box)
+        f_s = cs.aev_backward(g)
+        a_r = cr.aev_forward(pos, sp, w.box)
+        f_r = cr.aev_backward(g)
+        cs.check_status(); cr.check_status()
+        for which in (0, 1):
+            np.testing.assert_array_equal(cs.aev_export_pairs(which, cap=w.batch * w.n_atoms * 64),
+                                          cr.aev_export_pairs(which, cap=w.batch * w.n_atoms * 64))
+        # (the two contexts round displacements differently - wrapped position + image shift vs raw difference -
+        #  so they agree to fp32 rounding of the coordinates, inside north_star's bounds)
+        assert float((a_s - a_r).abs().max()) <= AEV_TOL * float(a_r.abs().max())
+        assert float((f_s - f_r).abs().max()) <= 5e-5 * float(f_r.abs().max())
+        if t in (0, 9, 19):
+            want_a = oracle.aev_forward(w.params, fr, w.species, w.box)
+            want_f = oracle.aev_backward(w.params, fr, w.species, w.box, w.grad_aev)
+            assert np.abs(a_s.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+            _check_forces(f_s.cpu().numpy(), want_f, what=("skin", kind, t))
+    builds = cs.neighbor_builds()
+    print("SKIN %s: %d builds in %d calls" % (kind, builds, len(frames)))
+    assert 2 <= builds <= 8
+    cs.close(); cr.close()
+
+
+def test_verlet_skin_inside_a_cuda_graph(pkg):
+    """The rebuild decision is taken on the device: one captured evaluation replayed over a trajectory (positions
+    updated in place) rebuilds when it must and matches the uncaptured context frame by frame."""
+    from gen import random_walk
+    w = make_water_box(216, 18.64, 311, "skin-graph")
+    frames = random_walk(w, 12, 0.05, 6)
+    cs = pkg.Context(w.params, max_atoms=w.n_atoms, skin=0.5)
+    cr = pkg.Context(w.params, max_atoms=w.n_atoms)
+    sp = torch.from_numpy(w.species).cuda()
+    g = torch.from_numpy(w.grad_aev).cuda()
+    pos = torch.from_numpy(w.pos).cuda()
+    aev = torch.empty((1, w.n_atoms, cs.length), dtype=torch.float32, device="cuda")
+    f = torch.empty((1, w.n_atoms, 3), dtype=torch.float32, device="cuda")
+
+    def step():
+        cs.aev_forward(pos, sp, w.box, aev_out=aev)
+        cs.aev_backward(g, forces_out=f)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.current_stream().wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        step()
+    b0 = cs.neighbor_builds()
+    for fr in frames:
+        pos.copy_(torch.from_numpy(fr).cuda())
+        graph.replay()
+        a_r = cr.aev_forward(pos, sp, w.box)
+        f_r = cr.aev_backward(g)
+        assert float((aev - a_r).abs().max()) <= 1e-5 * float(a_r.abs().max())
+        assert float((f - f_r).abs().max()) <= 5e-5 * float(f_r.abs().max())
+    cs.check_status()
+    builds = cs.neighbor_builds() - b0
+    assert 1 <= builds < len(frames)
+    del graph
+    cs.close(); cr.close()
