@@ -130,9 +130,16 @@ def _work_counts(counts: np.ndarray, pos: np.ndarray, box, rcr: float):
     return {"radial_pairs_directed": p_r, "angular_pairs_directed": p_a, "triplets": trip, "candidates": cand}
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on C4, from the one `ncu --set full` capture
-# summarised in profiles/r1_final_ncu_full.md (bench.py never runs under a profiler itself)
-NCU_TRAFFIC_BYTES = {"backward": 61.2e6 + 0.22e6, "aev": 25.4e6 + 0.42e6, "nbr": 0.96e6 + 0.18e6}
+def _ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch on C4, from the `ncu --set full` capture whose
+    summary is tracked as profiles/r2_ncu_traffic.json (written from the .ncu-rep, with the commit it was
+    measured at; bench.py never runs under a profiler itself).  ncu's default cache control flushes L2 before
+    every kernel, so these are COLD-CACHE bytes: inside a real step the neighbour lists are L2-resident."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_ncu_traffic.json")) as fh:
+            return json.load(fh)
+    except Exception:
+        return {}
 
 
 def _flops(wc):
@@ -152,10 +159,12 @@ def _oracle_eval(w, threads=None):
     oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=uc)
 
 
-def cpu_baseline(budget_s: float = 12.0):
+def cpu_baseline(budget_s: float = 10.0):
     """The oracle as it stands (fp64 C, OpenMP over central atoms, cell list) on this box's
-    host cores, on a bounded sample of the headline workload."""
+    host cores, on a bounded sample of the headline workload: full C4 evaluations on all cores, and
+    one on a single thread (both numbers and the CPU model are reported)."""
     import oracle
+    from oracle.build import cpu_model
     from gen import make_workload
     w = make_workload("C4")
     cores = oracle.max_threads()
@@ -167,34 +176,43 @@ def cpu_baseline(budget_s: float = 12.0):
         dt = time.perf_counter() - t0
         if dt > budget_s or n >= 8:
             break
+    t1 = time.perf_counter()
+    _oracle_eval(w, threads=1)
+    dt1 = time.perf_counter() - t1
+    oracle.set_threads(cores)
     return {"value": w.n_atoms * w.batch * n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "%d full C4 evaluations (fwd+bwd, fp64, cell list) in %.1f s" % (n, dt)}
+            "sample": "%d full C4 evaluations (fwd+bwd, fp64, cell list) in %.1f s on %d threads; 1 on one thread in %.1f s"
+                      % (n, dt, cores, dt1),
+            "value_1_thread": w.n_atoms * w.batch / dt1, "cpu_model": cpu_model().split(" [")[0],
+            "build": "gcc -O3 -march=native -ffp-contract=off -fopenmp (oracle/build.py)"}
 
 
 def run_reference(args):
-    """Reference arm of this tier: the oracle on the host cores; each step is one fwd+bwd
-    evaluation of a bounded sample of the workload (a 1,536-atom water box of the same
-    density and generator), so that K steps end within minutes."""
+    """Reference arm of this tier: the oracle on the host cores; each step is one full fwd+bwd
+    evaluation of the headline workload itself (C4; about 0.7 s on 16 cores, so K <= 200 steps end
+    within minutes)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
-    from gen import make_water_box
-    w = make_water_box(512, 61.7 * (512.0 / 7853.0) ** (1.0 / 3.0), 400, "C4-sample")
+    from oracle.build import cpu_model
+    from gen import make_workload
+    w = make_workload("C4")
     cores = oracle.max_threads()
-    for _ in range(max(1, min(args.warmup, 3))):
+    for _ in range(max(1, min(args.warmup, 2))):
         _oracle_eval(w)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         _oracle_eval(w)
     dt = time.perf_counter() - t0
     value = w.n_atoms * args.steps / dt
-    sample = "each step: fwd+bwd of a 1,536-atom water box (512 H2O, same density/generator as C4)"
+    sample = "each step: one full C4 evaluation (fwd+bwd, fp64, cell list) on %d threads of %s" % (
+        cores, cpu_model().split(" [")[0])
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "data": "synthetic", "config": {"workload": WORKLOAD, "atoms": w.n_atoms, "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -226,6 +244,37 @@ def _time_steps(fn, steps, flush, torch):
         e1.record()
     torch.cuda.synchronize()
     return np.array([e0.elapsed_time(e1) for e0, e1 in ev])
+
+
+def run_quick_c5(args):
+    """`--quick --workload C5|C5_ens8|C5_fp32`: only the full energy+forces evaluation (for ncu captures of k_mlp_tc)."""
+    import torch
+    import paper_2310_03121_b200 as pkg
+    from gen import make_ensemble_weights, make_workload
+    from gen.workloads import CELU_ALPHA
+    dev = torch.device("cuda", 0)
+    w5 = make_workload("C5")
+    models = {"C5": lambda: make_ensemble_weights(1), "C5_ens8": lambda: make_ensemble_weights(8),
+              "C5_fp32": lambda: make_ensemble_weights(1, round_bf16=False)}[args.workload]()
+    ctx = pkg.Context(w5.params, max_atoms=w5.n_atoms, device=0)
+    ctx.ani_mlp_set_ensemble(len(models))
+    for m, nets in enumerate(models):
+        for s, (ws, bs) in nets.items():
+            ctx.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
+    p5, s5 = torch.from_numpy(w5.pos).to(dev), torch.from_numpy(w5.species).to(dev)
+    e5 = torch.empty((1,), dtype=torch.float64, device=dev)
+    f5 = torch.empty((1, w5.n_atoms, 3), dtype=torch.float32, device=dev)
+    flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+
+    def st5():
+        ctx.ani_energy_forces(p5, s5, w5.box, energy_out=e5, forces_out=f5)
+    for _ in range(max(args.warmup, 3)):
+        st5()
+    tt = _time_steps(st5, args.steps, flush_buf.zero_, torch)
+    ctx.check_status()
+    print(json.dumps({"quick": True, "workload": args.workload, "ms_per_eval": float(tt.mean()),
+                      "atoms_per_s": w5.n_atoms / (tt.mean() * 1e-3), "mlp_kernel": ctx.mlp_kernel()}))
+    ctx.close()
 
 
 def run_ours(args):
@@ -315,7 +364,14 @@ def run_ours(args):
         probe = None
     roofline = {
         "bound": "alu", "kernel": "k_" + dom, "achieved": achieved, "peak": ALU_PEAK_TFLOPS,
-        "unit": "TFLOP/s", "frac": achieved / ALU_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(dom),
+        "unit": "TFLOP/s", "frac": achieved / ALU_PEAK_TFLOPS,
+        "traffic": (_ncu_traffic().get("k_" + dom) or {}).get("dram_bytes"),
+        "traffic_note": "ncu dram__bytes_read+write per launch, COLD cache (L2 flushed by ncu before the kernel); "
+                        "profiles/r2_ncu_traffic.json, measured at commit %s" % _ncu_traffic().get("commit"),
+        "algorithmic_bytes_per_launch": {"nbr": n_atoms * 16 + wc["radial_pairs_directed"] * 16,
+                                         "aev": n_atoms * ctx.length * 4 + wc["radial_pairs_directed"] * 16,
+                                         "backward": n_atoms * ctx.length * 4 + wc["radial_pairs_directed"] * 16
+                                         + n_atoms * 12}[dom],
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 7)",
         "fma_probe_tflops": probe,
         "algorithmic_flop_per_launch": dom_flop,
@@ -409,8 +465,48 @@ def run_ours(args):
     p5prof = c5.aev_get_profile()
     other["C5"] = {"ms_per_eval": float(tt.mean()), "atoms_per_s": w5.n_atoms / (tt.mean() * 1e-3),
                    "what": "ani_energy_forces: AEV + per-species MLP fwd/bwd + AEV backward, 4,500-atom box",
-                   "mlp_ms": p5prof["mlp"][0] / max(1, p5prof["mlp"][1])}
+                   "mlp_ms": p5prof["mlp"][0] / max(1, p5prof["mlp"][1]), "mlp_kernel": c5.mlp_kernel()}
+    c5.aev_set_profiling(False)
+    # the call an MD engine makes: positions in, energy + forces out, host buffers, synchronous
+    pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
+    p5h, s5h = pin(w5.pos), pin(w5.species)
+    for _ in range(3):
+        c5.ani_energy_forces_host(p5h, s5h, w5.box)
+    t0 = time.perf_counter()
+    n5 = 50
+    for _ in range(n5):
+        c5.ani_energy_forces_host(p5h, s5h, w5.box)
+    dt5 = (time.perf_counter() - t0) / n5
+    other["C5"]["e2e"] = {"ms_per_eval": dt5 * 1e3, "atoms_per_s": w5.n_atoms / dt5,
+                          "h2d_bytes_per_step": int(w5.pos.nbytes + w5.species.nbytes),
+                          "d2h_bytes_per_step": int(w5.n_atoms * 12 + 8),
+                          "call": "ani_energy_forces_host (wall clock, L2 not flushed)"}
     c5.close()
+
+    def c5_variant(models, tag, what):
+        cc = pkg.Context(w5.params, max_atoms=w5.n_atoms, device=local)
+        cc.ani_mlp_set_ensemble(len(models))
+        for m, nets in enumerate(models):
+            for s, (ws, bs) in nets.items():
+                cc.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
+
+        def stv():
+            cc.ani_energy_forces(p5, s5, w5.box, energy_out=e5, forces_out=f5)
+        for _ in range(3):
+            stv()
+        tv = _time_steps(stv, min(args.steps, 50), flush, torch)
+        cc.aev_set_profiling(True); cc.aev_get_profile()
+        for _ in range(5):
+            stv()
+        pv = cc.aev_get_profile()
+        other[tag] = {"ms_per_eval": float(tv.mean()), "atoms_per_s": w5.n_atoms / (tv.mean() * 1e-3), "what": what,
+                      "mlp_ms": pv["mlp"][0] / max(1, pv["mlp"][1]), "mlp_kernel": cc.mlp_kernel()}
+        cc.close()
+    from gen import make_ensemble_weights
+    c5_variant(make_ensemble_weights(8), "C5_ens8",
+               "C5 with an ensemble of 8 networks per species (PAPER.md:193), bf16-representable weights")
+    c5_variant(make_ensemble_weights(1, round_bf16=False), "C5_fp32_weights",
+               "C5 with fp32 (not bf16-representable) weights: weight hi+lo operands on tcgen05")
 
     cpu = cpu_baseline()
 
@@ -440,7 +536,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--quick", action="store_true",
                     help="headline loop + per-kernel pass only (for ncu runs): no e2e / other configs / cpu baseline")
+    ap.add_argument("--workload", default="C4", choices=["C4", "C5", "C5_ens8", "C5_fp32"],
+                    help="with --quick: C4 (headline step) or a C5 variant (full energy+forces evaluation)")
     args = ap.parse_args()
+    if args.quick and args.workload != "C4":
+        run_quick_c5(args)
+        return
     if args.impl == "reference":
         if args.steps > 200:
             args.steps = 200
