@@ -147,7 +147,15 @@ namespace aevb {
         if (e__ != cudaSuccess) return AEV_ERR_CUDA;      \
     } while (0)
 
-enum { kErrBitCapacity = 1, kErrBitState = 2 };
+enum { kErrBitCapacity = 1, kErrBitState = 2, kErrBitCheck = 4 };
+
+// -DAEVB_CHECKS (debug builds; compute-sanitizer is not available on every pool): bounds checks of the computed list
+// slots and shared-memory indices; a failed check raises kErrBitCheck, which aev_status reports as AEV_ERR_CUDA.
+#ifdef AEVB_CHECKS
+#define AEVB_CHECK(errp, cond) do { if (!(cond)) atomicOr((errp), kErrBitCheck); } while (0)
+#else
+#define AEVB_CHECK(errp, cond) do { } while (0)
+#endif
 
 // Every entry point runs on the context's device and leaves the caller's current device as it found it.
 class DeviceGuard {
