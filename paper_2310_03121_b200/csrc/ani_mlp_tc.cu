@@ -13,9 +13,12 @@
 // backward sweep (CELU' is recomputed from them); bias, CELU, the last (N = 1) layer, the
 // energy sum and the bf16 split run in the epilogue, one thread per row (tcgen05.ld 32x32b).
 //
-// Operand layout in shared memory (no swizzle, K-major "core matrices" of 8 rows x 16 bytes):
-//   element (r, k) of an [R x K] operand sits at  (k/8) * R*16 + r*16 + (k%8)*2  bytes,
-//   i.e. [K/8][R][8] bf16  =>  descriptor LBO = R*16 (next 8 k), SBO = 128 (next 8 rows).
+// Operand layout in shared memory: K-major, SWIZZLE_128B.  An [R x K] bf16 operand is cut into K blocks of 64
+// elements; block kb is R rows of 128 bytes (row r at kb*R*128 + r*128) and inside a row the 16-byte chunk c (8
+// elements) sits at chunk position c ^ (r & 7): the 8-row x 128-byte swizzle atoms the tensor core reads without
+// bank conflicts (descriptor: SBO = 1024 bytes between 8-row groups, layout type SWIZZLE_128B; one MMA consumes
+// K = 16 = 32 bytes, so the start address advances by 32 bytes per K step and by R*128 per block).  Atoms are
+// 1024-byte aligned.  The unswizzled "core matrix" layout of round 1 ran the MMAs at 2.8 x their floor.
 #include <cuda_bf16.h>
 #include <math.h>
 #include <stdio.h>
@@ -40,9 +43,10 @@ constexpr int kTM = 128;              // rows (atoms) per tile = MMA M
 constexpr int kTcGroups = 8;          // warpgroups per CTA: group g takes the 8-column chunks g, g+8, ... in the epilogues
 constexpr int kTcThreads = kTM * kTcGroups;
 constexpr int kKC = 64;               // K chunk of the first layer (AEV columns per stage)
-constexpr int kActBytes = 81920;      // activation operand: hi | lo, each up to [256/8... K<=160][128][8] bf16
+constexpr int kActBytes = 98304;      // activation operand: hi | lo, each up to 3 K blocks (K <= 192) of 128 rows x 128 bytes
 constexpr int kActHalf = kActBytes / 2;
-constexpr int kWBufBytes = 40960;     // one weight buffer (two of them, ping-pong)
+constexpr int kWBufBytes = 49152;     // one weight buffer (two of them, ping-pong): e.g. 3 K blocks x 128 rows x 128 bytes
+constexpr int kABlk = kTM * 128;      // bytes of one K block of the activation operand
 constexpr int kTcSmem = kActBytes + 2 * kWBufBytes + 1024;
 
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -94,11 +98,16 @@ __device__ __forceinline__ void tmem_ld8(unsigned taddr, float *v)      // no wa
 }
 __device__ __forceinline__ void tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// shared-memory matrix descriptor: no swizzle, K-major, version 1 (sm_100)
-__device__ __forceinline__ unsigned long long smem_desc(unsigned addr, unsigned lbo_bytes, unsigned sbo_bytes)
+// shared-memory matrix descriptor: K-major, SWIZZLE_128B (layout type 2 in bits 61-63), SBO = 1024 bytes, version 1
+// (sm_100); the leading-dimension offset is not used by swizzled K-major operands
+__device__ __forceinline__ unsigned long long smem_desc(unsigned addr)
 {
-    return (unsigned long long)((addr >> 4) & 0x3FFF) | ((unsigned long long)((lbo_bytes >> 4) & 0x3FFF) << 16) |
-           ((unsigned long long)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46);
+    return (unsigned long long)((addr >> 4) & 0x3FFF) | ((unsigned long long)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+// byte offset of the 16-byte chunk c (8 elements along K) of row r in an operand of R rows
+__device__ __forceinline__ unsigned sw_off(int r, int c, int R)
+{
+    return (unsigned)((c >> 3) * R * 128 + r * 128 + (((c & 7) ^ (r & 7)) << 4));
 }
 // instruction descriptor: kind::f16, A = B = bf16 (K-major), D = f32, M = 128, N = n
 __device__ __forceinline__ unsigned instr_desc(int n)
@@ -243,12 +252,14 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
         };
         auto load_w0 = [&](int kc) {      // stage kc of W_0: a contiguous block of the [K/8][N][8] operand
             const int kw = min(kKC, K0 - kc * kKC);
-            const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wf[0]) + (size_t)kc * (kKC / 8) * N1 * 16;
+            // K block kc of the packed operand: N1 rows x 128 bytes, already swizzled (a partial last block is zero-padded)
+            const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wf[0]) + (size_t)kc * N1 * 128;
             unsigned char *dst = wbuf[kc & 1];
-            const int pieces = (kw / 8) * N1;
+            const int pieces = 8 * N1;
+            (void)kw;
             for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
             if (need_lo) {      // residual operand: second half of the stage buffer
-                const unsigned char *srcl = src + (size_t)((K0 + 7) / 8) * N1 * 16;
+                const unsigned char *srcl = src + (size_t)((K0 + 63) / 64) * N1 * 128;
                 for (int t = tid; t < pieces; t += kTcThreads)
                     cp_async16_tc(dst + kWBufBytes / 2 + t * 16, srcl + (size_t)t * 16);
             }
@@ -264,8 +275,8 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
             if (grp < kw / 8) {          // this thread's k-chunk of the stage: columns kc*64 + grp*8 .. +7
                 uint4 hi, lo;
                 split8(x0.v, hi, lo);
-                *reinterpret_cast<uint4 *>(abuf + grp * 2048 + row * 16) = hi;
-                *reinterpret_cast<uint4 *>(abuf + 16384 + grp * 2048 + row * 16) = lo;
+                *reinterpret_cast<uint4 *>(abuf + sw_off(row, grp, kTM)) = hi;
+                *reinterpret_cast<uint4 *>(abuf + 16384 + sw_off(row, grp, kTM)) = lo;
             }
             x0 = x1;
             x1 = load_a(kc + 2);         // two stages ahead (zeros past the last stage)
@@ -277,12 +288,11 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
                 tc_fence_after();
                 const unsigned a_hi = smem_u32(abuf), a_lo = a_hi + 16384, b_a = smem_u32(wbuf[b]);
                 for (int ks = 0; ks < kw / 16; ++ks) {
-                    const unsigned long long bd = smem_desc(b_a + ks * 2 * N1 * 16, N1 * 16, 128);
-                    umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 4096, 2048, 128), bd, idesc, (kc | ks) != 0);
-                    umma_bf16(tmem + N.zoff[0], smem_desc(a_lo + ks * 4096, 2048, 128), bd, idesc, 1u);
+                    const unsigned long long bd = smem_desc(b_a + ks * 32);
+                    umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 32), bd, idesc, (kc | ks) != 0);
+                    umma_bf16(tmem + N.zoff[0], smem_desc(a_lo + ks * 32), bd, idesc, 1u);
                     if (need_lo)
-                        umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 4096, 2048, 128),
-                                  smem_desc(b_a + kWBufBytes / 2 + ks * 2 * N1 * 16, N1 * 16, 128), idesc, 1u);
+                        umma_bf16(tmem + N.zoff[0], smem_desc(a_hi + ks * 32), smem_desc(b_a + kWBufBytes / 2 + ks * 32), idesc, 1u);
                 }
                 umma_commit(&bar[b]);
             }
@@ -306,23 +316,23 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
     // whole-layer weight operand -> shared memory (contiguous [K/8][N][8] block; the residual operand right behind it)
     auto load_w = [&](const __nv_bfloat16 *w, int K, int Nn, unsigned char *dst) {
         const unsigned char *src = reinterpret_cast<const unsigned char *>(w);
-        const int pieces = (K / 8) * Nn * (need_lo ? 2 : 1);      // hi | lo are adjacent in global memory too
+        const int pieces = ((K + 63) / 64) * Nn * 8 * (need_lo ? 2 : 1);      // hi | lo are adjacent in global memory too
         for (int t = tid; t < pieces; t += kTcThreads) cp_async16_tc(dst + t * 16, src + (size_t)t * 16);
     };
-    // D[tmem + dcol] = act[128 x K] (hi + lo) * B[Nn x K]^T (hi [+ lo at wsm + K*Nn*2]), issued by one thread,
+    // D[tmem + dcol] = act[128 x K] (hi + lo) * B[Nn x K]^T (hi [+ lo behind the hi blocks]), issued by one thread,
     // completion on bar[2]
-    auto gemm = [&](int K, int Nn, const unsigned char *wsm, int lbo_b, unsigned dcol) {
+    auto gemm = [&](int K, int Nn, const unsigned char *wsm, unsigned dcol) {
         if (tid == 0) {
             tc_fence_after();
             const unsigned a_hi = smem_u32(act), a_lo = a_hi + kActHalf, b_a = smem_u32(wsm);
             const unsigned idesc = instr_desc(Nn);
+            const unsigned b_lo = b_a + ((K + 63) / 64) * Nn * 128;
             for (int ks = 0; ks < K / 16; ++ks) {
-                const unsigned long long bd = smem_desc(b_a + ks * 2 * lbo_b, lbo_b, 128);
-                umma_bf16(tmem + dcol, smem_desc(a_hi + ks * 4096, 2048, 128), bd, idesc, ks != 0);
-                umma_bf16(tmem + dcol, smem_desc(a_lo + ks * 4096, 2048, 128), bd, idesc, 1u);
-                if (need_lo)
-                    umma_bf16(tmem + dcol, smem_desc(a_hi + ks * 4096, 2048, 128),
-                              smem_desc(b_a + K * Nn * 2 + ks * 2 * lbo_b, lbo_b, 128), idesc, 1u);
+                const unsigned ao = (ks >> 2) * kABlk + (ks & 3) * 32, bo = (ks >> 2) * Nn * 128 + (ks & 3) * 32;
+                const unsigned long long bd = smem_desc(b_a + bo);
+                umma_bf16(tmem + dcol, smem_desc(a_hi + ao), bd, idesc, ks != 0);
+                umma_bf16(tmem + dcol, smem_desc(a_lo + ao), bd, idesc, 1u);
+                if (need_lo) umma_bf16(tmem + dcol, smem_desc(a_hi + ao), smem_desc(b_lo + bo), idesc, 1u);
             }
             umma_commit(&bar[2]);
         }
@@ -336,8 +346,8 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
     auto put8 = [&](const float *v, int c) {
         uint4 hi, lo;
         split8(v, hi, lo);
-        *reinterpret_cast<uint4 *>(act + c * 2048 + row * 16) = hi;
-        *reinterpret_cast<uint4 *>(act + kActHalf + c * 2048 + row * 16) = lo;
+        *reinterpret_cast<uint4 *>(act + sw_off(row, c, kTM)) = hi;
+        *reinterpret_cast<uint4 *>(act + kActHalf + sw_off(row, c, kTM)) = lo;
     };
     auto sync_for_mma = [&]() {      // generic-proxy writes + cp.async data visible to the tensor core
         cp_async_wait_all_tc();
@@ -393,7 +403,7 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
         }
         if (l < nh) {
             sync_for_mma();
-            gemm(Nl, N.dims[l + 1], wbuf[wsel], N.dims[l + 1] * 16, N.zoff[l]);
+            gemm(Nl, N.dims[l + 1], wbuf[wsel], N.zoff[l]);
             wsel ^= 1;
             wait_gemm();
         } else {
@@ -421,7 +431,7 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
         const int Kb = N.dims[l + 1], Nb = N.dims[l], ncl = Nb >> 3;
         const unsigned dcol = N.zoff[l];                   // z_(l+1) is dead: reuse its columns
         sync_for_mma();
-        gemm(Kb, Nb, wbuf[wsel], Nb * 16, dcol);
+        gemm(Kb, Nb, wbuf[wsel], dcol);
         if (!need_lo) {
             wsel ^= 1;
             if (l >= 2) load_w(N.wb[l - 1], Nb, N.dims[l - 1], wbuf[wsel]);   // next operand while the MMAs run
@@ -453,24 +463,26 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
     // ------------------------------------------------------------------ d_0 = d_1 W_0^T, N = L in chunks of CW
     {
         const int Kb = N.dims[1];
-        const int CW = need_lo ? 64 : 128;       // a chunk's hi (+ lo) operand fits one 40 KB buffer
+        const int CW = need_lo ? 64 : 128;       // a chunk's hi (+ lo) operand fits one 48 KB buffer
         const int nch = (L + CW - 1) / CW;
-        const size_t lo_off = (size_t)((Kb + 7) / 8) * L * 16;
+        const int nkb = (Kb + 63) / 64;
+        const size_t lo_off = (size_t)nkb * L * 128;
         if (need_lo) wsel = 0;
         auto load_chunk = [&](int j, unsigned char *dst) {
             const int n0 = j * CW, nw = min(CW, L - n0);
             const unsigned char *src = reinterpret_cast<const unsigned char *>(N.wb[0]);
-            const int pieces = (Kb / 8) * nw;
+            const int per = nw * 8, pieces = nkb * per;      // K block kb of the chunk: rows n0 .. n0+nw-1, 128 bytes each
             for (int t = tid; t < pieces; t += kTcThreads) {
-                const int kc = t / nw, n = t - kc * nw;
-                cp_async16_tc(dst + t * 16, src + ((size_t)kc * L + n0 + n) * 16);
-                if (need_lo) cp_async16_tc(dst + Kb * nw * 2 + t * 16, src + lo_off + ((size_t)kc * L + n0 + n) * 16);
+                const int kb = t / per, q = t - kb * per;
+                const size_t so = ((size_t)kb * L + n0) * 128 + (size_t)q * 16;
+                cp_async16_tc(dst + t * 16, src + so);
+                if (need_lo) cp_async16_tc(dst + pieces * 16 + t * 16, src + lo_off + so);
             }
         };
         // accumulators alternate between two TMEM slots (every z is dead by now): chunk j at column (j & 1) * 128
         load_chunk(0, wbuf[wsel]);
         sync_for_mma();
-        gemm(Kb, min(CW, L), wbuf[wsel], min(CW, L) * 16, 0u);
+        gemm(Kb, min(CW, L), wbuf[wsel], 0u);
         for (int j = 0; j < nch; ++j) {
             const int n0 = j * CW, nw = min(CW, L - n0);
             const unsigned slot = (unsigned)(j & 1) * 128u;
@@ -479,7 +491,7 @@ k_mlp_tc(const TcAll *__restrict__ Mg, int n_models, int L, int n_total, int n_a
             if (j + 1 < nch) {
                 const int nw1 = min(CW, L - (j + 1) * CW);
                 sync_for_mma();
-                gemm(Kb, nw1, wbuf[wsel ^ 1], nw1 * 16, slot ^ 128u);
+                gemm(Kb, nw1, wbuf[wsel ^ 1], slot ^ 128u);
                 wsel ^= 1;
             }
             // tcgen05.ld is warp-collective: rows without an atom take part, only the store is skipped
@@ -536,16 +548,19 @@ bool mlp_tc_eligible(const MlpNet &n, int L)
     const int nh = n.n_layers - 1;
     if (nh < 1 || nh > 3) return false;
     if (L % 16 || L > 4096 || n.dims[0] != L) return false;
-    const int wlim = n.bf16_exact ? kWBufBytes : 2 * kWBufBytes, per = n.bf16_exact ? 2 : 4;
+    const int wlim = n.bf16_exact ? kWBufBytes : 2 * kWBufBytes, per = n.bf16_exact ? 1 : 2;
     int off = 0;
     for (int l = 1; l <= nh; ++l) {
         if (n.dims[l] % 16 || n.dims[l] < 16 || n.dims[l] > 160) return false;
         off += n.dims[l];
     }
     if (off > 512) return false;
-    if (kKC * n.dims[1] * 2 > kWBufBytes / 2) return false;
-    for (int l = 1; l < nh; ++l)
-        if (n.dims[l] * n.dims[l + 1] * per > wlim) return false;
+    if (n.dims[1] * 128 > kWBufBytes / 2) return false;                       // one K block of W_0 (hi | lo halves)
+    for (int l = 1; l < nh; ++l) {                                            // inner layers, forward and backward operand
+        if (((n.dims[l] + 63) / 64) * n.dims[l + 1] * 128 * per > wlim) return false;
+        if (((n.dims[l + 1] + 63) / 64) * n.dims[l] * 128 * per > wlim) return false;
+    }
+    if (((n.dims[1] + 63) / 64) * 128 * 128 > kWBufBytes) return false;         // a 128- (64-) column chunk of W_0^T
     // backward accumulator of layer l reuses the columns from z_(l+1) on
     int zo = 0;
     for (int l = 1; l < nh; ++l) {
@@ -602,12 +617,18 @@ int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *a
     return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
 }
 
-// Host-side packing of one layer W[in][out] (row-major) into the two chunked operand layouts, each as the
-// bf16 hi parts followed by the bf16 residuals (w - hi) in the same layout.
+// Host-side packing of one layer W[in][out] (row-major) into the two swizzled K-major operand layouts (see the file
+// header), each as the bf16 hi parts followed by the bf16 residuals (w - hi) in the same layout:
+//   forward  operand B[n = out][k = in]:  K blocks of 64 inputs,  N_out rows of 128 bytes per block
+//   backward operand B[n = in][k = out]:  K blocks of 64 outputs, K_in  rows of 128 bytes per block
 void mlp_tc_pack(const float *w, int K_in, int N_out, std::vector<__nv_bfloat16> &fwd, std::vector<__nv_bfloat16> &bwd,
                  bool *exact)
 {
-    const size_t nf = (size_t)((K_in + 7) / 8) * N_out * 8, nb = (size_t)((N_out + 7) / 8) * K_in * 8;   // K padded to 8
+    auto idx = [](int row, int k, int rows) -> size_t {      // element index of (row, k) in an operand of `rows` rows
+        const int kb = k >> 6, c = (k & 63) >> 3;
+        return (size_t)kb * rows * 64 + (size_t)row * 64 + (size_t)((c ^ (row & 7)) << 3) + (k & 7);
+    };
+    const size_t nf = (size_t)((K_in + 63) / 64) * N_out * 64, nb = (size_t)((N_out + 63) / 64) * K_in * 64;
     fwd.assign(2 * nf, __float2bfloat16_rn(0.f));
     bwd.assign(2 * nb, __float2bfloat16_rn(0.f));
     bool ex = true;
@@ -617,11 +638,8 @@ void mlp_tc_pack(const float *w, int K_in, int N_out, std::vector<__nv_bfloat16>
             const __nv_bfloat16 b = __float2bfloat16_rn(v);
             const __nv_bfloat16 r = __float2bfloat16_rn(v - __bfloat162float(b));
             if (__bfloat162float(b) != v) ex = false;
-            // forward: B[n = o][kk = k]  ->  [kk/8][N_out][8]
-            const size_t fi = ((size_t)(k >> 3) * N_out + o) * 8 + (k & 7);
+            const size_t fi = idx(o, k, N_out), bi = idx(k, o, K_in);
             fwd[fi] = b; fwd[nf + fi] = r;
-            // backward: B[n = k][kk = o] ->  [kk/8][K_in][8]
-            const size_t bi = ((size_t)(o >> 3) * K_in + k) * 8 + (o & 7);
             bwd[bi] = b; bwd[nb + bi] = r;
         }
     *exact = ex;
