@@ -247,8 +247,8 @@ int aev_export_pairs(aev_ctx *c, int32_t which, int32_t *pairs_out, int64_t cap,
 int aev_export_counts(aev_ctx *c, int32_t *counts_out);
 /* Per-kernel device timing for bench.py's roofline: when enabled, every kernel launch is
  * bracketed by CUDA events on its stream.  aev_get_profile syncs, adds the elapsed times
- * since the last call to ms_out[0..4] = {bin, sort, aev, backward, nbr} plus
- * ms_out[5] = MLP, writes the launches seen per slot to n_out[0..5], and resets. */
+ * since the last call to ms_out[0..5] = {bin (k_bin, k_rank), fout (k_fout / k_fixout), aev (k_aev), backward (k_backward),
+ * nbr (k_nbr, k_refresh), mlp}, writes the launches seen per slot to n_out[0..5], and resets. */
 int aev_set_profiling(aev_ctx *c, int32_t enable);
 int aev_get_profile(aev_ctx *c, double *ms_out, int64_t *n_out);
 /* Syncs the context's last stream and returns AEV_OK or the deferred device-side error

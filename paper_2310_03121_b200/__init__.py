@@ -346,7 +346,7 @@ class Context:
         ms = (C.c_double * 6)()
         n = (C.c_int64 * 6)()
         _check(lib().aev_get_profile(self._h, ms, n), "aev_get_profile")
-        names = ("bin", "sort", "aev", "backward", "nbr", "mlp")
+        names = ("bin", "fout", "aev", "backward", "nbr", "mlp")
         return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(names)}
 
     def aev_status(self) -> int:

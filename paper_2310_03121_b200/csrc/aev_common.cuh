@@ -204,7 +204,8 @@ bool mlp_tc_eligible(const MlpNet &n, int L);
 int mlp_tc_upload(aev_ctx *c);
 int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *aev, float *grad_aev,
                             double *energy_out, cudaStream_t st);
-// profiling brackets (aev_kernels.cu): slot 0 bin, 1 sort, 2 aev (k_aev), 3 backward, 4 nbr (k_nbr), 5 mlp
+// profiling brackets (aev_kernels.cu): slot 0 bin (k_bin, k_rank), 1 fout (k_fout / k_fixout), 2 aev (k_aev), 3 backward,
+// 4 nbr (k_nbr, k_refresh), 5 mlp
 void prof_begin(aev_ctx *c, int slot, cudaStream_t st);
 void prof_end(aev_ctx *c, cudaStream_t st);
 
