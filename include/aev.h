@@ -71,9 +71,11 @@ typedef struct aev_ctx aev_ctx; /* opaque; owns all device workspace */
 
 /* aev_params.flags */
 enum {
-    AEV_FLAG_DETERMINISTIC = 1, /* aev_backward accumulates the force contributions on neighbours in
-                                   64-bit fixed point (2^-32 force units) instead of fp32 REDs: forces
-                                   are bit-identical run to run; a little slower  */
+    AEV_FLAG_DETERMINISTIC = 1, /* bit-identical AEV and forces run to run: the members of
+                                   every cell are ordered by atom index before the neighbour search (by default they
+                                   keep the order the binning atomics ran in, so AEV sums agree to rounding only),
+                                   and aev_backward accumulates the contributions on neighbours in 64-bit fixed point
+                                   (2^-32 force units) instead of fp32 REDs.  A little slower.                       */
     AEV_FLAG_MLP_FP32 = 2,      /* debugging: run the fp32 CUDA-core MLP kernel even where the tcgen05
                                    kernel qualifies                                                     */
     AEV_FLAG_TRICLINIC = 4      /* every `box` argument is HOST f32[9]: lattice vectors a, b, c as rows,
@@ -144,10 +146,11 @@ int aev_forward(aev_ctx *c, const float *pos, const int32_t *species, const floa
  *   forces_out  device f32 [batch][n_atoms][3], OVERWRITTEN,
  *               forces_out[a] = - sum_i sum_slot grad_aev[i][slot]*dAEV[i][slot]/dx_a
  * The centre's own terms are reduced with warp shuffles; the reaction on each radial
- * neighbour and the gradient on each angular neighbour are added with one fp32 RED per
- * component, so by default forces are reproducible to rounding, not bit for bit; with
+ * neighbour and the gradient on each angular neighbour are added with one 16-byte vector RED
+ * into a padded accumulator of the context (copied to forces_out and cleared by a last small
+ * kernel), so by default forces are reproducible to rounding, not bit for bit; with
  * AEV_FLAG_DETERMINISTIC they are accumulated in 64-bit fixed point and are bit-identical
- * run to run (the AEV itself always is while a cell's stencil fits the shared-memory stage,
+ * run to run (so is the AEV then, while a cell's stencil fits the shared-memory stage,
  * 1024 candidates).  AEV_ERR_STATE if no forward precedes it.  Asynchronous.
  */
 int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *stream);
