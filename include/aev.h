@@ -131,8 +131,8 @@ int aev_neighbors(aev_ctx *c, const float *pos, const int32_t *species, const fl
                   int32_t n_atoms, int32_t batch, void *stream);
 
 /*
- * Steps (1)-(3): neighbour search (always rebuilt, reading G18) + radial and
- * angular AEV (rows A1-A4).
+ * Steps (1)-(3): neighbour search (rebuilt in every call, reading G18, unless the context has a
+ * Verlet skin - see aev_params.skin) + radial and angular AEV (rows A1-A4).
  *   aev_out  device f32 [batch][n_atoms][L], OVERWRITTEN, rows in the caller's atom order;
  *            rows of padding atoms are written as zeros.
  * Keeps what aev_backward needs inside the context.  Asynchronous.
