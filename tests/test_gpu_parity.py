@@ -427,9 +427,10 @@ def test_cuda_graph_replay_with_new_positions(pkg):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("zeta", [8.0, 16.0])
-def test_other_power_of_two_zeta(pkg, zeta):
-    """zeta != 32 takes the run-time squaring-chain instantiations of k_aev / k_backward."""
+@pytest.mark.parametrize("zeta", [8.0, 16.0, 14.1, 1.0, 3.5])
+def test_other_zeta(pkg, zeta):
+    """zeta != 32: powers of two take the run-time squaring-chain instantiations of k_aev / k_backward, any other
+    value (14.1: the exponent the advisor recalls for published ANI-2x parameters) the exp2(zeta log2 b) ones."""
     import dataclasses
     w = make_workload("C2")
     p = dataclasses.replace(w.params, zeta=np.float32(zeta))
