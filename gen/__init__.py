@@ -10,6 +10,7 @@ PAPER.md:164 DHFR-sized solvated box) and rejects geometries that sit within
 from .workloads import (  # noqa: F401
     AniParams,
     ani1x_style_params,
+    ani2x_shaped_params,
     make_c1,
     make_c2,
     make_water_box,

@@ -73,6 +73,25 @@ def ani1x_style_params(cos_scale: float = 1.0, num_species: int = 4, dtype=np.fl
     )
 
 
+def ani2x_shaped_params(cos_scale: float = 1.0, num_species: int = 7) -> AniParams:
+    """The OTHER angular split the library supports - 8 angular radial shifts x 4 angle shifts, a zeta that is not
+    a power of two, 7 species (L = 1008) - with synthetic, evenly spaced shifts of this repository's own choosing
+    (the same ranges as the ANI-1x-style set): the SHAPE of a 2x-generation parameter set, not its published values."""
+    t = np.float32
+    return AniParams(
+        num_species=num_species,
+        rcr=t(5.2),
+        rca=t(3.5),
+        eta_r=t(16.0),
+        shf_r=np.linspace(0.9, 4.96875, 16).astype(np.float32),
+        eta_a=t(8.0),
+        zeta=t(14.1),
+        shf_a=np.linspace(0.9, 2.85, 8).astype(np.float32),
+        shf_z=((2.0 * np.arange(4) + 1.0) * math.pi / 8.0).astype(np.float32),
+        cos_scale=t(cos_scale),
+    )
+
+
 @dataclasses.dataclass
 class Workload:
     name: str

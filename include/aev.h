@@ -38,8 +38,8 @@
  *     capability 10.x gives AEV_ERR_UNSUPPORTED.
  *
  * Supported parameter space (else AEV_ERR_UNSUPPORTED): 1 <= num_species <= 8,
- * n_shf_r == 16, n_shf_a == 4, n_shf_z == 8 (the shift counts of BASELINE.json:configs[0],
- * "ANI-1x-style"; the lane mappings of the kernels are built on 16 / 4 x 8 = 32), 1 <= zeta <= 64
+ * n_shf_r == 16, (n_shf_a, n_shf_z) == (4, 8) - the shift counts of BASELINE.json:configs[0],
+ * "ANI-1x-style" - or (8, 4) (the lane mappings of the kernels are built on 16 and on 32 = 4 x 8 = 8 x 4), 1 <= zeta <= 64
  * (powers of two by repeated squaring, any other value - e.g. 14.1 - as exp2(zeta log2 b) on the SFU), 0 < rca <= rcr, 0 < cos_scale <= 1; periodic boxes are orthorhombic (three
  * edge lengths, each >= 2*rcr) or, with AEV_FLAG_TRICLINIC, reduced triclinic (three lattice
  * vectors, ax, by, cz >= 2*rcr).  Orthorhombic boxes with at least 3 cells of edge >= rcr along every

@@ -12,9 +12,10 @@
 namespace aevb {
 
 constexpr int kNR = 16;        // radial shifts   (BASELINE.json:configs[0])
-constexpr int kNA = 4;         // angular radial shifts
+constexpr int kNA = 4;         // angular radial shifts  (the ANI-1x-style default; 8 x 4 is the other supported split)
 constexpr int kNZ = 8;         // angular angle shifts
-constexpr int kBlk = kNA * kNZ;  // 32 entries per species-pair block
+constexpr int kBlk = kNA * kNZ;  // 32 entries per species-pair block, whatever the split
+constexpr int kMaxNA = 8, kMaxNZ = 8;
 constexpr int kMaxS = 8;
 constexpr int kSpeciesShift = 26;  // neighbour entry .w = caller index of j | species << 26
 constexpr int kIdxMask = (1 << kSpeciesShift) - 1;
@@ -24,6 +25,7 @@ constexpr int kMaxModels = 8;      // networks per species in an ensemble (PAPER
 // Everything the kernels need about the symmetry functions; passed by value (constant bank).
 struct DevParams {
     int S, L, rad_len, n_blocks, zeta_log2;
+    int n_a;                     // angular radial shifts: 4 (x 8 angle shifts) or 8 (x 4)
     float rcr, rca, rcr2, rca2;
     float eta_r, eta_a;          // natural units (for derivatives)
     float eta_r_l2, eta_a_l2;    // eta * log2(e)    (for ex2)
@@ -31,11 +33,11 @@ struct DevParams {
     float zeta_half;             // zeta / 2
     float c, c2, one_m_c2;       // cos_scale, its square, 1 - c^2
     float shf_r[kNR];
-    float shf_a[kNA];
-    float cz[kNZ], sz[kNZ];      // cos / sin of the angle shifts
+    float shf_a[kMaxNA];
+    float cz[kMaxNZ], sz[kMaxNZ];      // cos / sin of the angle shifts
     unsigned long long half2, neta_r2;                 // (0.5, 0.5) and (-eta_r log2 e) twice
     unsigned long long nshf_r2[kNR / 2];               // -shf_r, packed pairs (m even | m odd << 32)
-    unsigned long long hcz2[kNZ / 2], hsz2[kNZ / 2];   // cos/2, sin/2 of the angle shifts, packed pairs (z even | z odd << 32)
+    unsigned long long hcz2[kMaxNZ / 2], hsz2[kMaxNZ / 2];   // cos/2, sin/2 of the angle shifts, packed pairs (z even | z odd << 32)
 };
 
 // Geometry of one call (filled on the host per call, passed by value).

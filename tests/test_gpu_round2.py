@@ -340,3 +340,29 @@ def test_verlet_skin_inside_a_cuda_graph(pkg):
     assert 1 <= builds < len(frames)
     del graph
     cs.close(); cr.close()
+
+
+# --------------------------------------------------------------------------- the other angular split (8 x 4), zeta = 14.1
+@pytest.mark.parametrize("cos_scale", [1.0, 0.95])
+def test_eight_by_four_angular_split_with_general_zeta(pkg, cos_scale):
+    """8 angular radial shifts x 4 angle shifts, zeta = 14.1, 7 species (L = 1008): the templated lane mappings of
+    k_aev / k_backward (16 accumulators as 8 x 2 packed pairs) and the exp2(zeta log2 b) power, gas phase and periodic."""
+    from gen import ani2x_shaped_params
+    from test_gpu_parity import AEV_TOL
+    p = ani2x_shaped_params(cos_scale)
+    assert p.aev_length == 1008 and len(p.shf_a) == 8 and len(p.shf_z) == 4
+    rng = np.random.default_rng(78)
+    for name in ("C2", "C3"):
+        w = make_workload(name)
+        pos = w.pos[:4] if name == "C2" else w.pos
+        sp = rng.integers(0, 7, size=pos.shape[:2]).astype(np.int32)
+        g = rng.standard_normal(pos.shape[:2] + (1008,)).astype(np.float32)
+        ctx = pkg.Context(p, max_atoms=pos.shape[1], max_batch=pos.shape[0])
+        aev = ctx.aev_forward(torch.from_numpy(pos).cuda(), torch.from_numpy(sp).cuda(), w.box)
+        f = ctx.aev_backward(torch.from_numpy(g).cuda())
+        ctx.check_status()
+        want_a = oracle.aev_forward(p, pos, sp, w.box, use_cells=w.box is not None)
+        want_f = oracle.aev_backward(p, pos, sp, w.box, g, use_cells=w.box is not None)
+        assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+        _check_forces(f.cpu().numpy(), want_f, what=("8x4 split", name, cos_scale))
+        ctx.close()

@@ -379,6 +379,32 @@ def test_against_torch_autograd(cos_scale, periodic):
     assert np.count_nonzero(aev_o[:, 64:]) > 500     # the angular part is exercised
 
 
+def test_other_angular_split_and_general_zeta_against_torch_autograd():
+    """8 angular radial shifts x 4 angle shifts, zeta = 14.1, 7 species (L = 1008): the slot order a*nZ + z, the block
+    index and the pow() of the oracle with parameter counts other than the default, against the dense restatement."""
+    import torch
+    from gen import ani2x_shaped_params
+    p = ani2x_shaped_params(0.95)
+    rng = np.random.default_rng(22)
+    n = 9
+    while True:
+        pos = rng.uniform(0, 4.0, size=(n, 3)).astype(np.float32)
+        dd = pos[:, None] - pos[None]
+        if np.sqrt((dd ** 2).sum(-1))[np.triu_indices(n, 1)].min() > 0.8:
+            break
+    species = rng.integers(0, 7, size=n).astype(np.int32)
+    g = rng.standard_normal((1, n, 1008)).astype(np.float32)
+    x = torch.tensor(pos.astype(np.float64), requires_grad=True)
+    aev_t = _torch_aev(x, species, p, None)
+    assert aev_t.shape == (n, 1008)
+    (aev_t * torch.tensor(g[0].astype(np.float64))).sum().backward()
+    aev_o = oracle.aev_forward(p, pos[None], species[None], None)[0]
+    np.testing.assert_allclose(aev_o, aev_t.detach().numpy(), rtol=1e-11, atol=1e-14)
+    f_o = oracle.aev_backward(p, pos[None], species[None], None, g)[0]
+    np.testing.assert_allclose(f_o, -x.grad.numpy(), rtol=1e-9, atol=1e-11)
+    assert np.count_nonzero(aev_o[:, 112:]) > 300
+
+
 def test_cell_list_featurizer_equals_brute_force():
     w = make_c3()
     a = oracle.aev_forward(w.params, w.pos, w.species, w.box, use_cells=False)
