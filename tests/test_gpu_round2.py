@@ -366,3 +366,24 @@ def test_eight_by_four_angular_split_with_general_zeta(pkg, cos_scale):
         assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
         _check_forces(f.cpu().numpy(), want_f, what=("8x4 split", name, cos_scale))
         ctx.close()
+
+
+def test_wide_hidden_layers_run_the_cuda_core_kernel(pkg):
+    """Hidden widths above the tensor-core envelope (256 / 192 / 160: more than 512 TMEM columns) with the 8 x 4 split and
+    7 species: the fp32 CUDA-core kernel takes over (ani_mlp_kernel says so) within the fp32 force tolerance."""
+    from gen import ani2x_shaped_params
+    p = ani2x_shaped_params()
+    w = make_water_box(125, 15.6, 302, "wide-box")
+    rng = np.random.default_rng(71)
+    sp = rng.integers(0, 7, size=w.species.shape).astype(np.int32)
+    nets = make_c5_weights(seed=6, arch={s: [1008, 256, 192, 160, 1] for s in range(7)}, round_bf16=False)
+    ctx = pkg.Context(p, max_atoms=w.n_atoms)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    assert ctx.mlp_kernel() == "fp32"
+    e, f = ctx.ani_energy_forces(torch.from_numpy(w.pos).cuda(), torch.from_numpy(sp).cuda(), w.box)
+    ctx.check_status()
+    we, wf, _ = oracle.energy_forces(p, w.pos, sp, w.box, nets, CELU_ALPHA)
+    assert abs(float(e[0]) - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    _check_forces(f.cpu().numpy().astype(np.float64), wf, what="wide hidden layers")
+    ctx.close()
