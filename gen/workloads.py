@@ -363,20 +363,26 @@ CELU_ALPHA = 0.1
 
 
 def make_periodic_cell(n_atoms: int, cell, seed: int, name: str = "cell", cos_scale: float = 1.0,
-                       min_dist: float = 1.1) -> Workload:
+                       min_dist: float = 1.1, params: Optional[AniParams] = None) -> Workload:
     """`n_atoms` atoms of species H/C/N/O (uniform) at random positions in a small periodic cell
     (the ML region can itself be a periodic cell of a few hundred atoms).  `cell` is three
     edge lengths (orthorhombic) or a 3x3 matrix of lattice rows a, b, c (triclinic, reduced form).
     Atoms are drawn one by one in fractional coordinates and rejected if closer than `min_dist` to an
     earlier atom or within MARGIN of a cutoff (distances over the 27 nearest images, float64); a third of
     the atoms is then moved by whole lattice vectors so that positions lie outside the cell.
-    `Workload.box` is float32 [3] or [9] (lattice rows)."""
-    p = ani1x_style_params(cos_scale)
+    `Workload.box` is float32 [3] or [9] (lattice rows); `cell` None = a non-periodic cluster drawn in a 14 A cube.
+    `params` (default: the ANI-1x-style set) fixes the cutoffs of the margin test and the species count."""
+    p = ani1x_style_params(cos_scale) if params is None else params
+    periodic = cell is not None
+    if not periodic:
+        cell = [14.0, 14.0, 14.0]
     rng = np.random.default_rng(seed)
     cell = np.asarray(cell, dtype=np.float64)
     lat = np.diag(cell) if cell.size == 3 else cell.reshape(3, 3)
     lat = lat.astype(np.float32).astype(np.float64)
     shifts = np.array([[i, j, k] for i in (-1, 0, 1) for j in (-1, 0, 1) for k in (-1, 0, 1)], dtype=np.float64) @ lat
+    if not periodic:
+        shifts = np.zeros((1, 3))
     pos = np.zeros((0, 3))
     rcr, rca = float(p.rcr), float(p.rca)
     tries = 0
@@ -391,10 +397,11 @@ def make_periodic_cell(n_atoms: int, cell, seed: int, name: str = "cell", cos_sc
             if r.min() < min_dist or (np.abs(r - rcr) < 10 * MARGIN).any() or (np.abs(r - rca) < 10 * MARGIN).any():
                 continue
         pos = np.vstack([pos, x])
-    move = rng.random(n_atoms) < 0.33
-    pos = pos + np.where(move[:, None], rng.integers(-2, 3, size=(n_atoms, 3)).astype(np.float64) @ lat, 0.0)
-    species = rng.integers(0, 4, size=n_atoms).astype(np.int32)
-    box = (cell if cell.size == 3 else lat.reshape(9)).astype(np.float32)
+    if periodic:
+        move = rng.random(n_atoms) < 0.33
+        pos = pos + np.where(move[:, None], rng.integers(-2, 3, size=(n_atoms, 3)).astype(np.float64) @ lat, 0.0)
+    species = rng.integers(0, int(p.num_species), size=n_atoms).astype(np.int32)
+    box = None if not periodic else (cell if cell.size == 3 else lat.reshape(9)).astype(np.float32)
     return Workload(name, pos.astype(np.float32)[None], species[None], box,
                     _grad_aev((1, n_atoms, p.aev_length), seed), p)
 
