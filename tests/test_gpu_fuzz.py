@@ -67,3 +67,41 @@ def test_random_configuration(seed):
         else:
             assert not np.any(f.cpu().numpy())
     ctx.close()
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_network_shapes(seed):
+    """Random per-species architectures inside the tensor-core envelope (1-3 hidden layers, widths 16..160), ensembles
+    of 1-3 models, bf16-representable or fp32 weights, on a small periodic cell or a gas-phase cluster."""
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2310_03121_b200 as pkg
+    from gen import make_c5_weights
+    from gen.workloads import CELU_ALPHA
+    from test_gpu_parity import C5_FORCE_MAX_TOL, C5_FORCE_TOL
+    rng = np.random.default_rng(2000 + seed)
+    S = int(rng.integers(1, 5))
+    p = ani1x_style_params(num_species=S)
+    cell = [None, (12.0, 13.0, 14.5), (17.0, 16.5, 18.0)][seed % 3]
+    n = int(rng.integers(40, 220))
+    w = make_periodic_cell(n, cell, 7000 + seed, params=p)
+    L = p.aev_length
+    arch = {}
+    for s in range(S):
+        nh = int(rng.integers(1, 4))
+        arch[s] = [L] + [int(16 * rng.integers(1, 11)) for _ in range(nh)] + [1]
+    n_models = int(rng.integers(1, 4))
+    exact = bool(seed % 2)
+    models = [make_c5_weights(seed=40 + seed + 10 * m, arch=arch, round_bf16=exact) for m in range(n_models)]
+    ctx = pkg.Context(p, max_atoms=n)
+    ctx.ani_mlp_set_ensemble(n_models)
+    for m, nets in enumerate(models):
+        for s, (ws, bs) in nets.items():
+            ctx.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
+    assert ctx.mlp_kernel() == "tcgen05", arch
+    e, f = ctx.ani_energy_forces(torch.from_numpy(w.pos).cuda(), torch.from_numpy(w.species).cuda(), w.box)
+    ctx.check_status()
+    we, wf, _ = oracle.energy_forces_ensemble(p, w.pos, w.species, w.box, models, CELU_ALPHA)
+    assert abs(float(e[0]) - we[0]) <= 1e-4 * max(1.0, abs(we[0])), (arch, n_models)
+    _check_forces(f.cpu().numpy().astype(np.float64), wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what=("net fuzz", seed, arch, n_models, exact))
+    ctx.close()
