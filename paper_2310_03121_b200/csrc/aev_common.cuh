@@ -139,6 +139,13 @@ struct aev_ctx {
     void *d_stage; size_t d_stage_bytes;
     cudaStream_t s_main, s_h2d, s_d2h;      // streams of the host entry points (kernels, big H2D, big D2H)
     cudaEvent_t ev_fwd, ev_grad;
+    // ani_energy_forces_host: the whole evaluation (H2D, kernels, D2H) as a CUDA graph, captured on the second call
+    // with the same shapes and box and replayed from then on (an MD engine calls it every step: 13 enqueue calls -> 1)
+    cudaGraphExec_t hg_exec;
+    int hg_state;                // 0: nothing seen, 1: one eager call with this key seen, 2: graph ready, -1: capture failed
+    int hg_n, hg_batch, hg_boxn;
+    float hg_box[9];
+    int64_t hg_launches;         // kernels per replay
 };
 
 namespace aevb {

@@ -296,6 +296,8 @@ extern "C" int ani_mlp_set_ensemble(aev_ctx *c, int32_t n_models)
     for (int m = 0; m < kMaxModels; ++m)
         for (int s = 0; s < kMaxS; ++s) free_net(c->nets[m][s]);
     c->n_models = n_models;
+    if (c->hg_exec) { cudaGraphExecDestroy(c->hg_exec); c->hg_exec = nullptr; }
+    c->hg_state = 0;      // a captured host-call graph has the old networks baked in
     return AEV_OK;
 }
 
@@ -322,6 +324,8 @@ extern "C" int ani_mlp_load_model(aev_ctx *c, int32_t model, int32_t species, in
     DeviceGuard guard(c->device);
     if (!guard.ok()) return AEV_ERR_CUDA;
     AEVB_CUDA(cudaDeviceSynchronize());
+    if (c->hg_exec) { cudaGraphExecDestroy(c->hg_exec); c->hg_exec = nullptr; }
+    c->hg_state = 0;      // a captured host-call graph has the old networks baked in
     MlpNet &n = c->nets[model][species];
     free_net(n);
     n.n_layers = n_layers;
