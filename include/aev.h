@@ -222,10 +222,14 @@ int ani_energy_forces_subset(aev_ctx *c, const float *pos_all, const int32_t *ml
  * pointer is a HOST pointer; the library stages through pinned buffers and device
  * workspace it owns, runs the same kernels, and copies the results back.  They sync.
  * Any of aev_out / grad_aev+forces_out may be NULL to skip that half.
- * Page-locked host buffers (cudaHostAlloc, cudaHostRegister, torch pin_memory) are copied from /
- * to directly; pageable ones are staged through the context's pinned buffer.  The copy of
- * grad_aev, the forward kernels and the read-back of aev_out run on three streams of the
- * context, so the two PCIe directions overlap each other and the kernels.
+ * aev_forward_backward_host: page-locked host buffers (cudaHostAlloc, cudaHostRegister, torch pin_memory) are copied
+ * from / to directly, pageable ones are staged through the context's pinned buffer.  Positions and species go up first,
+ * then the copy of grad_aev, the forward kernels and the read-back of aev_out run on three streams of the context, so
+ * the two PCIe directions overlap each other and the kernels.
+ * ani_energy_forces_host (the call an MD engine makes every step): inputs and results pass through the
+ * context's pinned buffer, which the kernels read and write directly over PCIe (no copy operations); from the second
+ * call with the same n_atoms, batch and box on, the whole evaluation is one replayed CUDA graph.
+ * Both return deferred device-side errors (AEV_ERR_CAPACITY, AEV_ERR_STATE) themselves.
  */
 int aev_forward_backward_host(aev_ctx *c, const float *pos, const int32_t *species,
                               const float *box, int32_t n_atoms, int32_t batch,
