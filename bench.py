@@ -502,7 +502,26 @@ def run_ours(args):
         other[tag] = {"ms_per_eval": float(tv.mean()), "atoms_per_s": w5.n_atoms / (tv.mean() * 1e-3), "what": what,
                       "mlp_ms": pv["mlp"][0] / max(1, pv["mlp"][1]), "mlp_kernel": cc.mlp_kernel()}
         cc.close()
+    # the paper's own ML workload shape: one 60-atom ligand-like region per MD step, host call
     from gen import make_ensemble_weights
+    wl = make_workload("C2")
+    lig = {}
+    for nm in (1, 8):
+        cl = pkg.Context(wl.params, max_atoms=wl.n_atoms, device=local)
+        cl.ani_mlp_set_ensemble(nm)
+        for m, nets in enumerate(make_ensemble_weights(nm, arch={s: [384, 160, 128, 96, 1] for s in range(4)})):
+            for s, (ws, bs) in nets.items():
+                cl.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
+        lp, ls = np.ascontiguousarray(wl.pos[:1]), np.ascontiguousarray(wl.species[:1])
+        for _ in range(5):
+            cl.ani_energy_forces_host(lp, ls, None)
+        t0 = time.perf_counter()
+        for _ in range(300):
+            cl.ani_energy_forces_host(lp, ls, None)
+        lig["models_%d_us_per_call" % nm] = (time.perf_counter() - t0) / 300 * 1e6
+        cl.close()
+    lig["what"] = "ani_energy_forces_host on one 60-atom conformer of C2 (host positions in, energy + forces out, wall clock)"
+    other["ligand_md_step"] = lig
     c5_variant(make_ensemble_weights(8), "C5_ens8",
                "C5 with an ensemble of 8 networks per species (PAPER.md:193), bf16-representable weights")
     c5_variant(make_ensemble_weights(1, round_bf16=False), "C5_fp32_weights",
