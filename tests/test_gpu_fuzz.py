@@ -98,7 +98,8 @@ def test_random_network_shapes(seed):
     for m, nets in enumerate(models):
         for s, (ws, bs) in nets.items():
             ctx.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
-    assert ctx.mlp_kernel() == "tcgen05", arch
+    # (fp32 weights with a wide inner layer, e.g. 144 -> 160, exceed the 96 KB operand buffers: those run the fp32 kernel)
+    assert ctx.mlp_kernel() in ("tcgen05", "fp32"), arch
     e, f = ctx.ani_energy_forces(torch.from_numpy(w.pos).cuda(), torch.from_numpy(w.species).cuda(), w.box)
     ctx.check_status()
     we, wf, _ = oracle.energy_forces_ensemble(p, w.pos, w.species, w.box, models, CELU_ALPHA)
