@@ -387,3 +387,38 @@ def test_wide_hidden_layers_run_the_cuda_core_kernel(pkg):
     assert abs(float(e[0]) - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
     _check_forces(f.cpu().numpy().astype(np.float64), wf, what="wide hidden layers")
     ctx.close()
+
+
+def test_host_call_graph_survives_reallocation_and_other_calls(pkg):
+    """ani_energy_forces_host replays a captured CUDA graph from the second call with one key on; a call that makes the
+    context reallocate workspace (a periodic box after gas-phase calls), other shapes and a network reload in between
+    must not leave a stale graph behind."""
+    w = make_workload("C2")
+    box_w = make_water_box(216, 18.64, 312, "graph-box")
+    nets = make_c5_weights(seed=3, arch={s: [384, 96, 64, 1] for s in range(4)})
+    ctx = pkg.Context(w.params, max_atoms=box_w.n_atoms)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    pos, sp = np.ascontiguousarray(w.pos[:1]), np.ascontiguousarray(w.species[:1])
+    want_e, want_f, _ = oracle.energy_forces(w.params, pos, sp, None, nets, CELU_ALPHA)
+
+    def check(n_calls):
+        for _ in range(n_calls):
+            e, f = ctx.ani_energy_forces_host(pos, sp, None)
+            assert abs(e[0] - want_e[0]) <= 1e-4 * max(1.0, abs(want_e[0]))
+            _check_forces(f.astype(np.float64), want_f, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what="host graph")
+    check(4)                                                   # eager, capture, replay, replay
+    eb, fb = ctx.ani_energy_forces_host(box_w.pos, box_w.species, box_w.box)      # other key; bin tables are allocated
+    wbe, wbf, _ = oracle.energy_forces(box_w.params, box_w.pos, box_w.species, box_w.box, nets, CELU_ALPHA)
+    _check_forces(fb.astype(np.float64), wbf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what="host call, box")
+    check(4)
+    pos2 = np.ascontiguousarray(w.pos[1:2])                    # same key, new positions: the replay reads the staging buffer
+    e2, f2 = ctx.ani_energy_forces_host(pos2, sp, None)
+    we2, wf2, _ = oracle.energy_forces(w.params, pos2, sp, None, nets, CELU_ALPHA)
+    _check_forces(f2.astype(np.float64), wf2, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what="host graph, new positions")
+    nets2 = make_c5_weights(seed=4, arch={s: [384, 96, 64, 1] for s in range(4)})
+    for s, (ws, bs) in nets2.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)                # reload: the graph with the old networks is dropped
+    want_e, want_f, _ = oracle.energy_forces(w.params, pos, sp, None, nets2, CELU_ALPHA)
+    check(3)
+    ctx.close()
