@@ -422,3 +422,25 @@ def test_host_call_graph_survives_reallocation_and_other_calls(pkg):
     want_e, want_f, _ = oracle.energy_forces(w.params, pos, sp, None, nets2, CELU_ALPHA)
     check(3)
     ctx.close()
+
+
+@pytest.mark.parametrize("flags,skin", [(0, 0.0), (1, 0.0), (0, 0.5), (1, 0.5)])
+def test_host_call_over_a_trajectory_in_every_mode(pkg, flags, skin):
+    """ani_energy_forces_host (replayed CUDA graph from the second call on) over an 8-frame random walk, default /
+    deterministic contexts with and without a Verlet skin (the rebuild decision is taken inside the replayed graph)."""
+    from gen import random_walk
+    w = make_water_box(216, 18.64, 320, "host-modes")
+    nets = make_c5_weights()
+    frames = random_walk(w, 8, 0.05, 9)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, flags=flags, skin=skin)
+    for s, (ws, bs) in nets.items():
+        ctx.ani_mlp_load(s, ws, bs, CELU_ALPHA)
+    for t, fr in enumerate(frames):
+        e, f = ctx.ani_energy_forces_host(np.ascontiguousarray(fr), w.species, w.box)
+        if t in (0, 1, 2, 7):
+            we, wf, _ = oracle.energy_forces(w.params, fr, w.species, w.box, nets, CELU_ALPHA, use_cells=True)
+            assert abs(e[0] - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+            _check_forces(f.astype(np.float64), wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what=("host modes", flags, skin, t))
+    if skin > 0:
+        assert 1 <= ctx.neighbor_builds() < len(frames)
+    ctx.close()
