@@ -64,7 +64,9 @@ enum {
                                    on the device; results of that call are incomplete          */
     AEV_ERR_STATE = -4,         /* aev_backward without a preceding aev_forward, MLP not loaded */
     AEV_ERR_UNSUPPORTED = -5,   /* parameter combination or device outside the supported space  */
-    AEV_ERR_CUDA = -6           /* a CUDA runtime call failed                                   */
+    AEV_ERR_CUDA = -6,          /* a CUDA runtime call failed                                   */
+    AEV_ERR_STATIC_LIMIT = -7   /* aev_pairs_static: more atoms than its fixed, statically allocated working
+                                   memory holds (AEV_STATIC_MAX_ATOMS); use a context instead    */
 };
 
 typedef struct aev_ctx aev_ctx; /* opaque; owns all device workspace */
@@ -237,6 +239,41 @@ int aev_forward_backward_host(aev_ctx *c, const float *pos, const int32_t *speci
 int ani_energy_forces_host(aev_ctx *c, const float *pos, const int32_t *species,
                            const float *box, int32_t n_atoms, int32_t batch,
                            double *energy_out, float *forces_out);
+
+/*
+ * Pair search that allocates nothing (step (1), rows A1-A2, "building neighbor lists"), for one
+ * non-periodic system such as the gas-phase ML region of PAPER.md:183-215 (53 ML atoms).
+ *
+ * Why it exists: every call above needs an aev_ctx, and a context gets its workspace from cudaMalloc (in
+ * aev_create, and again whenever a call brings larger shapes).  That is not an option for a host that gave the
+ * whole GPU to its own memory pool at start-up, for a step loop that cannot afford the device-wide
+ * synchronisation cudaMalloc / cudaFree imply, or for a component whose device-memory footprint has to be known
+ * when it is linked.  This call takes no context and never calls cudaMalloc, cudaFree or any library routine
+ * that allocates: its only working memory (one int per atom) is an array compiled into the library, 16 KB that
+ * every GPU loading libaev_b200.so holds until the process exits.  The price is a hard size limit.
+ *
+ *   pos        device f32 [n_atoms][3]
+ *   species    device i32 [n_atoms], or NULL = every atom is real; id < 0 = padding atom (in no pair)
+ *   n_atoms    0 .. AEV_STATIC_MAX_ATOMS; more returns AEV_ERR_STATIC_LIMIT and launches nothing (the array
+ *              cannot grow - use aev_neighbors + aev_export_pairs on a context for larger systems)
+ *   rc         cutoff, > 0; a pair is listed when r_ij < rc (strict; same fp32 test as aev_neighbors, so the
+ *              set equals the one aev_export_pairs returns for the same system, bit for bit)
+ *   pairs_out  device i32 [cap][2], pairs (i < j) SORTED by i, then j (aev_export_pairs promises no order)
+ *   count_out  DEVICE i64 [1] = pairs found; may exceed cap, then only the first cap (in that order) are written
+ *   device     CUDA ordinal the pointers live on; the caller's current device is restored on return
+ *   stream     as everywhere.  Asynchronous; nothing is read back to the host.
+ *
+ * First call on a device: it looks up the device address of the array once (no allocation, but the runtime may
+ * have to load the module), so make one call per device during start-up, before any stream capture begins.
+ * Sharing: the array belongs to the device, not to a caller, and keeps the previous call's contents.  No part
+ * of it has to be cleared - each call overwrites the n_atoms entries it later reads - but two calls that can
+ * run at the same time on one GPU (different streams with no event between them, or different host threads)
+ * overwrite each other's counts and both results are garbage.  Issue them on one stream or order them with
+ * events.
+ */
+#define AEV_STATIC_MAX_ATOMS 4096
+int aev_pairs_static(const float *pos, const int32_t *species, int32_t n_atoms, float rc,
+                     int32_t *pairs_out, int64_t cap, int64_t *count_out, int32_t device, void *stream);
 
 /*
  * Test / diagnostic exports.

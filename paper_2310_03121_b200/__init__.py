@@ -23,14 +23,15 @@ LIB_PATH = os.path.join(_HERE, "libaev_b200.so")
 AEV_OK = 0
 ERRORS = {
     -1: "AEV_ERR_INVALID_ARG", -2: "AEV_ERR_BOX_TOO_SMALL", -3: "AEV_ERR_CAPACITY",
-    -4: "AEV_ERR_STATE", -5: "AEV_ERR_UNSUPPORTED", -6: "AEV_ERR_CUDA",
+    -4: "AEV_ERR_STATE", -5: "AEV_ERR_UNSUPPORTED", -6: "AEV_ERR_CUDA", -7: "AEV_ERR_STATIC_LIMIT",
 }
+AEV_STATIC_MAX_ATOMS = 4096      # include/aev.h
 
 EXPORTS = [
     "aev_create", "aev_destroy", "aev_length", "aev_neighbors", "aev_forward", "aev_backward",
     "ani_mlp_load", "ani_mlp_set_ensemble", "ani_mlp_load_model", "ani_mlp_kernel", "ani_energy_forces", "ani_energy_forces_subset", "aev_forward_backward_host", "ani_energy_forces_host",
     "aev_export_pairs", "aev_export_counts", "aev_set_profiling", "aev_get_profile", "aev_status", "aev_launch_count", "aev_neighbor_builds", "aev_probe_fp32_tflops",
-    "aev_error_string",
+    "aev_error_string", "aev_pairs_static",
 ]
 
 
@@ -124,6 +125,8 @@ def lib():
         L.aev_launch_count.argtypes = [vp]
         L.aev_probe_fp32_tflops.restype = C.c_int
         L.aev_probe_fp32_tflops.argtypes = [i32, C.POINTER(C.c_double)]
+        L.aev_pairs_static.restype = C.c_int
+        L.aev_pairs_static.argtypes = [f32p, i32p, i32, C.c_float, i32p, i64, vp, i32, vp]
         L.aev_error_string.restype = C.c_char_p
         L.aev_error_string.argtypes = [C.c_int]
         _lib = L
@@ -362,6 +365,29 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().aev_launch_count(self._h))
+
+
+def aev_pairs_static(pos, species, rc: float, pairs_out, count_out, stream=None) -> None:
+    """Pair search of one non-periodic system without any device allocation (include/aev.h, aev_pairs_static).
+
+    For callers that must not allocate on the GPU (the device belongs to their own pool, their step loop cannot
+    take the synchronisation cudaMalloc brings, or their footprint is fixed at link time): no context, and the
+    library's working memory is a fixed array inside the .so.  So this wrapper allocates nothing either - the
+    caller brings every buffer: `pos` f32 [n, 3], `species` i32 [n] or None, `pairs_out` i32 [cap, 2],
+    `count_out` i64 [1], all CUDA tensors on one device.  On return (asynchronously, on the current stream)
+    `count_out[0]` pairs (i < j, r < rc) sit in `pairs_out`, sorted by (i, j).  n > AEV_STATIC_MAX_ATOMS raises
+    AevError(AEV_ERR_STATIC_LIMIT).  One call per GPU at a time: all calls on a device share that array.
+    """
+    import torch
+    n = int(pos.shape[0])
+    if pos.dim() != 2 or pos.shape[1] != 3:
+        raise TypeError("pos must be [n_atoms, 3]")
+    sp = None if species is None else _dev_ptr(species, torch.int32, "species")
+    cap = int(pairs_out.shape[0])
+    _check(lib().aev_pairs_static(_dev_ptr(pos, torch.float32, "pos"), sp, n, float(rc),
+                                  _dev_ptr(pairs_out, torch.int32, "pairs_out"), cap,
+                                  _dev_ptr(count_out, torch.int64, "count_out"), int(pos.device.index or 0),
+                                  _stream(stream)), "aev_pairs_static")
 
 
 def probe_fp32_tflops(device: int = 0) -> float:

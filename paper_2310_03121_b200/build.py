@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libaev_b200.so")
-SOURCES = ["aev_kernels.cu", "ani_mlp.cu", "ani_mlp_tc.cu"]
+SOURCES = ["aev_kernels.cu", "ani_mlp.cu", "ani_mlp_tc.cu", "aev_static.cu"]
 HEADERS = ["aev_common.cuh", os.path.join("..", "..", "include", "aev.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
