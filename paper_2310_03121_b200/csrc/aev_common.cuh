@@ -146,6 +146,7 @@ struct aev_ctx {
     int hg_n, hg_batch, hg_boxn;
     float hg_box[9];
     int64_t hg_launches;         // kernels per replay
+    aevb::Geom hg_geom, hg_vgeom; // c->geom / c->vgeom as the captured evaluation left them (restored after every replay)
 };
 
 namespace aevb {
