@@ -5,6 +5,7 @@
 #include <math.h>
 #include <string.h>
 
+#include <memory>
 #include <vector>
 
 #include "aev_common.cuh"
@@ -215,7 +216,9 @@ int mlp_group(aev_ctx *c, const int32_t *species, int n_total, int batch, double
 // Device table of the fp32 kernel; rebuilt whenever a network is (re)loaded.  Syncs.
 static int mlp_f32_upload(aev_ctx *c)
 {
-    static MlpAll M;      // 8 KB: not on the stack
+    // 8 KB, built on the heap per call: two contexts may load networks from two host threads at once
+    std::unique_ptr<MlpAll> Mp(new MlpAll);
+    MlpAll &M = *Mp;
     memset(&M, 0, sizeof(M));
     for (int m = 0; m < c->n_models; ++m)
         for (int s = 0; s < c->dp.S; ++s) {

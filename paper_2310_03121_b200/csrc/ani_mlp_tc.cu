@@ -24,6 +24,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <memory>
 #include <vector>
 
 #include "aev_common.cuh"
@@ -574,7 +575,9 @@ bool mlp_tc_eligible(const MlpNet &n, int L)
 int mlp_tc_upload(aev_ctx *c)
 {
     const int S = c->dp.S;
-    static TcAll M;      // 9 KB: not on the stack
+    // 9 KB, built on the heap per call: two contexts may load networks from two host threads at once
+    std::unique_ptr<TcAll> Mp(new TcAll);
+    TcAll &M = *Mp;
     memset(&M, 0, sizeof(M));
     for (int m = 0; m < c->n_models; ++m)
         for (int s = 0; s < S; ++s) {
