@@ -165,10 +165,14 @@ int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *str
  *            row-major ("[in][out]")
  *   biases   HOST array of n_layers HOST pointers, f32 [dims[l+1]]
  * Hidden activations are CELU(alpha); the last layer is linear.  Syncs.
- * Which kernel runs: hidden widths <= 160 with the pre-activations of all hidden layers fitting
- * 512 TMEM columns take the tcgen05 kernel (activations AND weights as bf16 hi + lo operands:
- * hi*hi + lo*hi + hi*lo, fp32 accumulate; the weight-lo MMA is skipped for a network whose
- * weights are all bf16-representable); other shapes run the fp32 CUDA-core kernel.
+ * Which kernel runs (ani_mlp_kernel tells): the tcgen05 kernel takes a network with 1-3 hidden layers of width
+ * 16..160 whose pre-activations fit the 512 TMEM columns (the hidden widths sum to <= 512, and for every hidden
+ * layer l but the last, width_1 + .. + width_l + width_l <= 512: its backward accumulator sits behind z_1..z_l) and
+ * whose inner-layer weight operands each fit one 48 KB shared-memory buffer, forward and transposed: for consecutive
+ * hidden widths (a, b), ceil(a/64)*b <= 384 and ceil(b/64)*a <= 384 - so 128 -> 160 and 160 -> 128 qualify,
+ * 144 -> 160 and 160 -> 160 do not.  Activations AND weights go in as bf16 hi + lo operands (hi*hi + lo*hi + hi*lo,
+ * fp32 accumulate; the weight-lo MMA is skipped for a network whose weights are all bf16-representable).  Any other
+ * shape, or any loaded network outside the envelope, makes the whole evaluation run the fp32 CUDA-core kernel.
  * ani_mlp_load == ani_mlp_load_model with model = 0 of an ensemble of 1.
  */
 int ani_mlp_load(aev_ctx *c, int32_t species, int32_t n_layers, const int32_t *dims,

@@ -60,3 +60,49 @@ def test_host_graph_replay_on_a_skin_context_after_a_call_with_other_shapes(pkg)
     host_call("replay again")
     assert ctx.neighbor_builds() == builds + 2           # nothing moved: the lists are reused
     ctx.close()
+
+
+@pytest.mark.parametrize("zeta", [1.0, 1.5, 32.0])
+@pytest.mark.parametrize("name", ["line3", "grid9"])
+def test_collinear_triplets_where_the_angular_base_is_exactly_zero(pkg, name, zeta):
+    """8 x 4 angular split (always the exp2(zeta log2 b) kernels) with angle shifts 0 and pi and cos_scale = 1: an
+    exactly collinear triplet makes b = (1 + cos(theta - shf_z))/2 exactly 0.  The backward needs b^(zeta-1) there:
+    1 for zeta = 1 (computed as ex2(0 * lg2(0)) it would be NaN), 0 otherwise."""
+    import dataclasses
+    from gen import ani2x_shaped_params
+    from test_gpu_edge_cases import _collinear_systems
+    from test_gpu_parity import AEV_TOL
+    pos, sp = _collinear_systems()[name]
+    p = dataclasses.replace(ani2x_shaped_params(1.0, num_species=4), zeta=np.float32(zeta),
+                            shf_z=np.array([0.0, np.pi / 3, 2 * np.pi / 3, np.pi], dtype=np.float32))
+    g = np.random.default_rng(6).standard_normal((1, len(sp), p.aev_length)).astype(np.float32)
+    ctx = pkg.Context(p, max_atoms=len(sp))
+    aev = ctx.aev_forward(torch.from_numpy(pos[None]).cuda(), torch.from_numpy(sp[None]).cuda(), None)
+    f = ctx.aev_backward(torch.from_numpy(g).cuda())
+    ctx.check_status()
+    want_a = oracle.aev_forward(p, pos[None], sp[None], None)
+    want_f = oracle.aev_backward(p, pos[None], sp[None], None, g)
+    assert np.isfinite(f.cpu().numpy()).all()
+    assert np.abs(aev.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+    _check_forces(f.cpu().numpy(), want_f, what=(name, zeta))
+    ctx.close()
+
+
+@pytest.mark.parametrize("round_bf16", [True, False])
+def test_kernel_choice_follows_the_documented_envelope(pkg, round_bf16):
+    """include/aev.h (ani_mlp_load) states which shapes run on the tensor cores; ani_mlp_kernel must agree, for
+    bf16-representable and for fp32 weights alike (hi + lo operands get two buffers, so the rule is the same)."""
+    from gen import ani1x_style_params
+    from test_gpu_fuzz import _in_tensor_core_envelope
+    p = ani1x_style_params(num_species=1)
+    L = p.aev_length
+    cases = {(160, 128, 96): "tcgen05", (128, 160): "tcgen05", (160, 128): "tcgen05", (144, 128): "tcgen05",
+             (144, 160): "fp32", (160, 160): "fp32", (96, 160, 160): "fp32", (176,): "fp32", (256, 192, 160): "fp32"}
+    for hidden, want in cases.items():
+        dims = [L] + list(hidden) + [1]
+        assert _in_tensor_core_envelope(dims) == (want == "tcgen05"), hidden      # the restated rule itself
+        nets = make_c5_weights(seed=11, arch={0: dims}, round_bf16=round_bf16)
+        ctx = pkg.Context(p, max_atoms=8)
+        ctx.ani_mlp_load(0, nets[0][0], nets[0][1], CELU_ALPHA)
+        assert ctx.mlp_kernel() == want, (hidden, round_bf16)
+        ctx.close()
