@@ -77,7 +77,10 @@ enum {
                                    every cell are ordered by atom index before the neighbour search (by default they
                                    keep the order the binning atomics ran in, so AEV sums agree to rounding only),
                                    and aev_backward accumulates the contributions on neighbours in 64-bit fixed point
-                                   (2^-32 force units) instead of fp32 REDs.  A little slower.                       */
+                                   (2^-32 force units) instead of fp32 REDs; with an ensemble the networks run as one
+                                   launch per model, so the mean dE/dAEV - and the forces of ani_energy_forces - are
+                                   summed in model order.  Energies are fp64 atomic sums and agree to fp64 rounding
+                                   only.  A little slower.                                                          */
     AEV_FLAG_MLP_FP32 = 2,      /* debugging: run the fp32 CUDA-core MLP kernel even where the tcgen05
                                    kernel qualifies                                                     */
     AEV_FLAG_TRICLINIC = 4      /* every `box` argument is HOST f32[9]: lattice vectors a, b, c as rows,

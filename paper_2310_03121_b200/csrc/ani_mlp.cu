@@ -265,6 +265,15 @@ int mlp_forward_backward(aev_ctx *c, const int32_t *species, int n_total, int n_
     }
     if (!c->f32_dev) return AEV_ERR_STATE;
     dim3 grid((n_total + TM - 1) / TM, S, nm);
+    if ((c->hp.flags & AEV_FLAG_DETERMINISTIC) && nm > 1) {      // one launch per model: the models' adds arrive in model order
+        grid.z = 1;
+        for (int m = 0; m < nm; ++m) {
+            const MlpAll *row = reinterpret_cast<const MlpAll *>(static_cast<const MlpAll *>(c->f32_dev)->net + m);
+            launch_pdl(k_mlp_f32<TM>, grid, dim3(256), smem, st, row, nm, L, n_total, n_atoms,
+                       (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->ws.err);
+        }
+        c->launches += nm - 1;
+    } else
     launch_pdl(k_mlp_f32<TM>, grid, dim3(256), smem, st, static_cast<const MlpAll *>(c->f32_dev), nm, L, n_total, n_atoms,
                (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->ws.err);
     prof_end(c, st);

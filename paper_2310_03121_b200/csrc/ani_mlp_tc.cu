@@ -615,6 +615,19 @@ int mlp_tc_forward_backward(aev_ctx *c, int n_total, int n_atoms, const float *a
         c->tc_smem_optin = 1;
     }
     dim3 grid((n_total + kTM - 1) / kTM, S, c->n_models);
+    if ((c->hp.flags & AEV_FLAG_DETERMINISTIC) && c->n_models > 1) {
+        // bit-reproducible mean dE/dAEV: one launch per model, so the fp32 REDs of the models land on every element in
+        // model order (within one launch each element is added to once); grid.z = 1 and the table pointer advanced
+        // to model m's row, so that blockIdx.z = 0 addresses it
+        grid.z = 1;
+        for (int m = 0; m < c->n_models; ++m) {
+            const TcAll *row = reinterpret_cast<const TcAll *>(static_cast<const TcAll *>(c->tc_dev)->net + m);
+            launch_pdl(k_mlp_tc, grid, dim3(kTcThreads), (size_t)kTcSmem, st, row, c->n_models, L, n_total, n_atoms,
+                       (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->ws.err);
+        }
+        c->launches += c->n_models - 1;
+        return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;
+    }
     launch_pdl(k_mlp_tc, grid, dim3(kTcThreads), (size_t)kTcSmem, st, static_cast<const TcAll *>(c->tc_dev), c->n_models, L,
                n_total, n_atoms, (const int *)c->sp_rows, (const int *)c->sp_count, aev, grad_aev, energy_out, c->ws.err);
     return cudaGetLastError() == cudaSuccess ? AEV_OK : AEV_ERR_CUDA;

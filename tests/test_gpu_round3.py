@@ -106,3 +106,73 @@ def test_kernel_choice_follows_the_documented_envelope(pkg, round_bf16):
         ctx.ani_mlp_load(0, nets[0][0], nets[0][1], CELU_ALPHA)
         assert ctx.mlp_kernel() == want, (hidden, round_bf16)
         ctx.close()
+
+
+@pytest.mark.parametrize("flags", [1, 1 | 2])
+def test_deterministic_ensemble_forces_are_bit_identical(pkg, flags):
+    """AEV_FLAG_DETERMINISTIC with an ensemble: the mean dE/dAEV is accumulated over the models in model order (one MLP
+    launch per model), so ani_energy_forces returns bit-identical forces run to run - on the tensor-core kernel and
+    (flag 2) on the fp32 kernel - and they still match the oracle."""
+    from gen import make_ensemble_weights, make_water_box
+    w = make_water_box(216, 18.64, 300, "det-ens")
+    models = make_ensemble_weights(3)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, flags=flags)
+    ctx.ani_mlp_set_ensemble(len(models))
+    for m, nets in enumerate(models):
+        for s, (ws, bs) in nets.items():
+            ctx.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
+    assert ctx.mlp_kernel() == ("fp32" if flags & 2 else "tcgen05")
+    pos, sp = torch.from_numpy(w.pos).cuda(), torch.from_numpy(w.species).cuda()
+    runs = []
+    for _ in range(4):
+        e, f = ctx.ani_energy_forces(pos, sp, w.box)
+        runs.append((e.clone(), f.clone()))
+    ctx.check_status()
+    for e, f in runs[1:]:
+        assert torch.equal(f, runs[0][1])
+    we, wf, _ = oracle.energy_forces_ensemble(w.params, w.pos, w.species, w.box, models, CELU_ALPHA, use_cells=True)
+    assert abs(float(runs[0][0][0]) - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    _check_forces(runs[0][1].cpu().numpy().astype(np.float64), wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what=("det ens", flags))
+    ctx.close()
+
+
+def test_c4_in_a_deterministic_context(pkg):
+    """The headline workload (23,559 atoms, cell list) under AEV_FLAG_DETERMINISTIC: k_rank's per-bin ordering and the
+    fixed-point accumulator at full size; AEV and forces bit-identical over two runs and within the oracle tolerances."""
+    from test_gpu_parity import AEV_TOL
+    w = make_workload("C4")
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, flags=pkg.AEV_FLAG_DETERMINISTIC)
+    pos, sp, g = (torch.from_numpy(x).cuda() for x in (w.pos, w.species, w.grad_aev))
+    a1 = ctx.aev_forward(pos, sp, w.box).clone()
+    f1 = ctx.aev_backward(g).clone()
+    a2 = ctx.aev_forward(pos, sp, w.box)
+    f2 = ctx.aev_backward(g)
+    ctx.check_status()
+    assert torch.equal(a1, a2) and torch.equal(f1, f2)
+    want_a = oracle.aev_forward(w.params, w.pos, w.species, w.box, use_cells=True)
+    want_f = oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=True)
+    assert np.abs(a1.cpu().numpy() - want_a).max() <= AEV_TOL * np.abs(want_a).max()
+    _check_forces(f1.cpu().numpy(), want_f, what="C4 deterministic")
+    ctx.close()
+
+
+def test_c4_with_a_verlet_skin(pkg):
+    """C4 with skin = 0.5 over three frames of a random walk: the Verlet capacities (vcap_r) at full size; pair sets
+    bit-exact against the oracle and forces within tolerance at every frame, lists reused at least once."""
+    from gen import random_walk
+    w = make_workload("C4")
+    frames = random_walk(w, 3, 0.02, 11)
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms, skin=0.5)
+    sp, g = torch.from_numpy(w.species).cuda(), torch.from_numpy(w.grad_aev).cuda()
+    for t, fr in enumerate(frames):
+        fr = np.ascontiguousarray(fr)
+        ctx.aev_forward(torch.from_numpy(fr).cuda(), sp, w.box)
+        f = ctx.aev_backward(g)
+        ctx.check_status()
+        got = ctx.aev_export_pairs(0, cap=w.n_atoms * 40)
+        np.testing.assert_array_equal(got, oracle.pairs(fr[0], w.species[0], w.box, float(w.params.rcr), "cell"))
+        if t in (0, 2):
+            want_f = oracle.aev_backward(w.params, fr, w.species, w.box, w.grad_aev, use_cells=True)
+            _check_forces(f.cpu().numpy(), want_f, what=("C4 skin", t))
+    assert 1 <= ctx.neighbor_builds() < len(frames)
+    ctx.close()
