@@ -70,13 +70,13 @@ def lib():
     and a compiler is present).  Raises if it cannot be had: there is no fallback."""
     global _lib
     if _lib is None:
-        path = LIB_PATH
-        try:
-            from .build import build
-            path = build()
-        except Exception:
-            if not os.path.exists(LIB_PATH):
-                raise
+        from .build import build, compiler_present
+        if compiler_present():
+            path = build()          # a failed compile raises: never fall back to a library built from older sources
+        elif os.path.exists(LIB_PATH):
+            path = LIB_PATH         # no nvcc on this machine: use the library that was shipped with the tree
+        else:
+            raise RuntimeError("libaev_b200.so is missing and there is no nvcc to build it (no fallback exists)")
         L = C.CDLL(path)
         vp, i32, i64, f32p, i32p = C.c_void_p, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p
         L.aev_create.restype = C.c_int

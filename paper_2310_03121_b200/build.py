@@ -24,10 +24,19 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _nvcc() -> str:
+    return os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+
+
+def compiler_present() -> bool:
+    import shutil
+    return shutil.which(_nvcc()) is not None
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    nvcc = _nvcc()
     tmp = LIB + ".tmp%d" % os.getpid()
     extra = os.environ.get("AEVB_NVCC_EXTRA", "").split()      # e.g. -DAEVB_TC_TIMING for debug builds
     cmd = [nvcc] + NVCC_FLAGS + extra + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES] + ["-lcudart"]

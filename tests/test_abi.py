@@ -75,3 +75,17 @@ def test_sass_has_no_local_memory_spill_in_hot_kernels():
                 assert int(st) == 0 and int(ld) == 0, "%s spills: %s B stores / %s B loads" % (key, st, ld)
     missing = [k for k, n in hot.items() if n == 0]
     assert not missing, "hot kernels not found in the ptxas log: %s" % missing
+
+
+def test_a_failed_build_is_not_hidden_by_an_older_library(monkeypatch):
+    """If the sources changed and nvcc fails, loading must raise instead of silently using the previous binary."""
+    import paper_2310_03121_b200 as pkg
+    import paper_2310_03121_b200.build as b
+    assert b.compiler_present()
+    assert os.path.exists(pkg.LIB_PATH)
+    monkeypatch.setattr(pkg, "_lib", None)
+    monkeypatch.setattr(b, "_stale", lambda: True)
+    monkeypatch.setattr(b, "NVCC_FLAGS", b.NVCC_FLAGS + ["--no-such-nvcc-flag"])
+    with pytest.raises(RuntimeError):
+        pkg.lib()
+    assert os.path.exists(pkg.LIB_PATH)      # the old library is left alone, just not loaded
