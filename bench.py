@@ -187,6 +187,16 @@ def cpu_baseline(budget_s: float = 10.0):
             "build": "gcc -O3 -march=native -ffp-contract=off -fopenmp (oracle/build.py)"}
 
 
+def _config(n_atoms):
+    """The `config` object both arms print, key for key (the driver compares them): what the workload is and how
+    each arm is timed.  Per-run details (ranks, core count, sample) are in the line's `arm` object."""
+    return {"workload": WORKLOAD, "atoms": int(n_atoms),
+            "l2": "GPU arm: flushed before every timed step (256 MiB memset outside the event pair); "
+                  "reference arm: CPU, not applicable",
+            "timing": "GPU arm: per-step CUDA events on the launching stream, summed, max over ranks; "
+                      "reference arm: wall clock on rank 0"}
+
+
 def run_reference(args):
     """Reference arm of this tier: the oracle on the host cores; each step is one full fwd+bwd
     evaluation of the headline workload itself (C4; about 0.7 s on 16 cores, so K <= 200 steps end
@@ -212,7 +222,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": WORKLOAD, "atoms": w.n_atoms, "sample": sample},
+        "data": "synthetic", "config": _config(w.n_atoms), "arm": {"parallelism": "host threads x%d" % cores, "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -368,10 +378,12 @@ def run_ours(args):
         "traffic": (_ncu_traffic().get("k_" + dom) or {}).get("dram_bytes"),
         "traffic_note": "ncu dram__bytes_read+write per launch, COLD cache (L2 flushed by ncu before the kernel); "
                         "profiles/r2_ncu_traffic.json, measured at commit %s" % _ncu_traffic().get("commit"),
-        "algorithmic_bytes_per_launch": {"nbr": n_atoms * 16 + wc["radial_pairs_directed"] * 16,
-                                         "aev": n_atoms * ctx.length * 4 + wc["radial_pairs_directed"] * 16,
-                                         "backward": n_atoms * ctx.length * 4 + wc["radial_pairs_directed"] * 16
-                                         + n_atoms * 12}[dom],
+        # the AEV / gradient matrix and the per-atom arrays are algorithmic; the neighbour lists are an
+        # implementation choice and are listed separately (cold-cache `traffic` contains both)
+        "algorithmic_bytes_per_launch": {"nbr": n_atoms * 16, "aev": n_atoms * ctx.length * 4 + n_atoms * 16,
+                                         "backward": n_atoms * ctx.length * 4 + n_atoms * 28}[dom],
+        "list_bytes_per_launch": wc["radial_pairs_directed"] * 16,
+        "frac_vs_probe": (achieved / probe) if probe else None,
         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 7)",
         "fma_probe_tflops": probe,
         "algorithmic_flop_per_launch": dom_flop,
@@ -446,6 +458,23 @@ def run_ours(args):
         except Exception as exc:      # reported, never fatal for the headline
             other[name]["graph_error"] = repr(exc)[:200]
         c2.close()
+    # the headline step in the two optional context modes (same buffers; include/aev.h: flags, skin)
+    for tag, kw, what in (("C4_deterministic", {"flags": pkg.AEV_FLAG_DETERMINISTIC},
+                           "C4 step with AEV_FLAG_DETERMINISTIC (k_rank + fixed-point force accumulator)"),
+                          ("C4_skin", {"skin": 0.5},
+                           "C4 step on a Verlet-skin context (skin 0.5), positions unchanged between calls: every timed "
+                           "step reuses the lists (k_disp + k_refresh instead of k_bin + k_nbr)")):
+        cm = pkg.Context(w.params, max_atoms=w.n_atoms, max_batch=w.batch, device=local, **kw)
+
+        def stm():
+            cm.aev_forward(pos, sp, w.box, aev_out=aev_out)
+            cm.aev_backward(g, forces_out=f_out)
+        for _ in range(3):
+            stm()
+        tm = _time_steps(stm, min(args.steps, 50), flush, torch)
+        cm.check_status()
+        other[tag] = {"ms_per_eval": float(tm.mean()), "atoms_per_s": n_atoms / (tm.mean() * 1e-3), "what": what}
+        cm.close()
     w5 = make_workload("C5")
     c5 = pkg.Context(w5.params, max_atoms=w5.n_atoms, device=local)
     for s, (ws, bs) in make_c5_weights().items():
@@ -533,10 +562,9 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": WORKLOAD, "atoms": n_atoms, "parallelism": "replicas x%d" % world,
-                   "l2": "flushed before every timed step (256 MiB memset outside the event pair)",
-                   "timing": "per-step CUDA events on the launching stream, summed; max over ranks",
-                   "ms_per_step_median": float(np.median(t_ms)), "ms_per_step_min": float(t_ms.min())},
+        "config": _config(n_atoms),
+        "arm": {"parallelism": "replicas x%d" % world, "ms_per_step_median": float(np.median(t_ms)),
+                "ms_per_step_min": float(t_ms.min())},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roofline, "cpu_baseline": cpu, "other": other,
     }

@@ -155,8 +155,9 @@ int aev_forward(aev_ctx *c, const float *pos, const int32_t *species, const floa
  * into a padded accumulator of the context (copied to forces_out and cleared by a last small
  * kernel), so by default forces are reproducible to rounding, not bit for bit; with
  * AEV_FLAG_DETERMINISTIC they are accumulated in 64-bit fixed point and are bit-identical
- * run to run (so is the AEV then, while a cell's stencil fits the shared-memory stage,
- * 1024 candidates).  AEV_ERR_STATE if no forward precedes it.  Asynchronous.
+ * run to run (so is the AEV then: every cell is searched in atom-index order, whether its
+ * stencil fits the shared-memory stage or is scanned from global memory).
+ * AEV_ERR_STATE if no forward precedes it.  Asynchronous.
  */
 int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *stream);
 

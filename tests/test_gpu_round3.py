@@ -176,3 +176,52 @@ def test_c4_with_a_verlet_skin(pkg):
             _check_forces(f.cpu().numpy(), want_f, what=("C4 skin", t))
     assert 1 <= ctx.neighbor_builds() < len(frames)
     ctx.close()
+
+
+def test_ensemble_of_three_seven_species_models_on_the_tensor_cores(pkg):
+    """Ensemble x L = 1008 together: three models per species of a seven-species set, so the
+    mean dE/dAEV is built by vector REDs over 8 column chunks per model; tcgen05 kernel, oracle tolerances of C5."""
+    from gen import ani1x_style_params, make_water_box
+    from gen.workloads import C5_ARCH
+    p7 = ani1x_style_params(num_species=7)
+    w = make_water_box(216, 18.64, 303, "s7-ens")
+    sp = np.random.default_rng(71).integers(0, 7, size=w.species.shape).astype(np.int32)
+    arch = {s: [1008] + C5_ARCH[0 if s % 2 == 0 else 3][1:] for s in range(7)}
+    models = [make_c5_weights(seed=20 + m, arch=arch, round_bf16=(m != 1)) for m in range(3)]
+    ctx = pkg.Context(p7, max_atoms=w.n_atoms)
+    ctx.ani_mlp_set_ensemble(3)
+    for m, nets in enumerate(models):
+        for s, (ws, bs) in nets.items():
+            ctx.ani_mlp_load_model(m, s, ws, bs, CELU_ALPHA)
+    assert ctx.mlp_kernel() == "tcgen05"
+    e, f = ctx.ani_energy_forces(torch.from_numpy(w.pos).cuda(), torch.from_numpy(sp).cuda(), w.box)
+    ctx.check_status()
+    we, wf, _ = oracle.energy_forces_ensemble(p7, w.pos, sp, w.box, models, CELU_ALPHA, use_cells=True)
+    assert abs(float(e[0]) - we[0]) <= 1e-4 * max(1.0, abs(we[0]))
+    _check_forces(f.cpu().numpy().astype(np.float64), wf, C5_FORCE_TOL, C5_FORCE_MAX_TOL, what="S=7 ensemble of 3")
+    ctx.close()
+
+
+def test_deterministic_flag_on_the_unstaged_neighbour_scan(pkg):
+    """A 1,200-atom gas-phase cluster is one cell whose candidates exceed the shared-memory stage, so k_nbr scans global
+    memory with warp ballots.  Under AEV_FLAG_DETERMINISTIC that scan reads the cell in atom-index order (k_rank), so
+    lists, AEV and forces are bit-identical run to run here too, and match the oracle."""
+    from gen import make_water_box
+    from test_gpu_parity import AEV_TOL
+    wb = make_water_box(400, 24.0, 910, "cluster")
+    pos, sp, g = (torch.from_numpy(x).cuda() for x in (wb.pos, wb.species, wb.grad_aev))
+    ctx = pkg.Context(wb.params, max_atoms=wb.n_atoms, flags=pkg.AEV_FLAG_DETERMINISTIC)
+    runs = []
+    for _ in range(3):
+        a = ctx.aev_forward(pos, sp, None).clone()
+        runs.append((a, ctx.aev_backward(g).clone()))
+    ctx.check_status()
+    for a, f in runs[1:]:
+        assert torch.equal(a, runs[0][0]) and torch.equal(f, runs[0][1])
+    got = ctx.aev_export_pairs(0, cap=wb.n_atoms * 64)
+    np.testing.assert_array_equal(got, oracle.pairs(wb.pos[0], wb.species[0], None, float(wb.params.rcr), "brute"))
+    want_aev = oracle.aev_forward(wb.params, wb.pos, wb.species, None, use_cells=False)
+    want_f = oracle.aev_backward(wb.params, wb.pos, wb.species, None, wb.grad_aev, use_cells=False)
+    assert np.abs(runs[0][0].cpu().numpy() - want_aev).max() <= AEV_TOL * np.abs(want_aev).max()
+    _check_forces(runs[0][1].cpu().numpy(), want_f, what="unstaged, deterministic")
+    ctx.close()
