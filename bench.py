@@ -132,11 +132,11 @@ def _work_counts(counts: np.ndarray, pos: np.ndarray, box, rcr: float):
 
 def _ncu_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch on C4, from the `ncu --set full` capture whose
-    summary is tracked as profiles/r2_ncu_traffic.json (written from the .ncu-rep, with the commit it was
+    summary is tracked as profiles/r3_ncu_traffic.json (written from the .ncu-rep, with the commit it was
     measured at; bench.py never runs under a profiler itself).  ncu's default cache control flushes L2 before
     every kernel, so these are COLD-CACHE bytes: inside a real step the neighbour lists are L2-resident."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_ncu_traffic.json")) as fh:
+        with open(os.path.join(ROOT, "profiles", "r3_ncu_traffic.json")) as fh:
             return json.load(fh)
     except Exception:
         return {}
@@ -377,7 +377,7 @@ def run_ours(args):
         "unit": "TFLOP/s", "frac": achieved / ALU_PEAK_TFLOPS,
         "traffic": (_ncu_traffic().get("k_" + dom) or {}).get("dram_bytes"),
         "traffic_note": "ncu dram__bytes_read+write per launch, COLD cache (L2 flushed by ncu before the kernel); "
-                        "profiles/r2_ncu_traffic.json, measured at commit %s" % _ncu_traffic().get("commit"),
+                        "profiles/r3_ncu_traffic.json, measured at commit %s" % _ncu_traffic().get("commit"),
         # the AEV / gradient matrix and the per-atom arrays are algorithmic; the neighbour lists are an
         # implementation choice and are listed separately (cold-cache `traffic` contains both)
         "algorithmic_bytes_per_launch": {"nbr": n_atoms * 16, "aev": n_atoms * ctx.length * 4 + n_atoms * 16,
