@@ -162,6 +162,23 @@ int aev_forward(aev_ctx *c, const float *pos, const int32_t *species, const floa
 int aev_backward(aev_ctx *c, const float *grad_aev, float *forces_out, void *stream);
 
 /*
+ * A slab of the central atoms (sharding the evaluation over GPUs; the paper's only
+ * parallelism content is multi-GPU MD over NVLink).  aev_forward_range is aev_forward for
+ * the central atoms with flat index (b*n_atoms + a) in [first, first + count) only: the neighbour search still
+ * covers every atom (a slab's neighbours lie outside it), but only the AEV rows of the slab are computed and
+ * written - every other row of aev_out is left untouched.  The aev_backward that follows then reads grad_aev
+ * rows [first, first + count) only and returns the PARTIAL forces
+ *     forces_out[a] = - sum_{i in slab} sum_slot grad_aev[i][slot] * dAEV[i][slot]/dx_a      for ALL atoms a,
+ * so the partial forces of disjoint slabs that cover the system add up to aev_backward's forces (to fp32 rounding).
+ * One process per GPU evaluates its slab on the full position array and the partial forces are summed across ranks
+ * (paper_2310_03121_b200/sharded.py: all-reduce over NCCL).  AEV_ERR_INVALID_ARG if the range is empty or leaves
+ * [0, batch*n_atoms).  The range applies to this call and its aev_backward only.  Asynchronous.
+ */
+int aev_forward_range(aev_ctx *c, const float *pos, const int32_t *species, const float *box,
+                      int32_t n_atoms, int32_t batch, int32_t first, int32_t count, float *aev_out,
+                      void *stream);
+
+/*
  * Loads the network of one species (rows A8-A9; BASELINE.json:configs[4]).
  *   dims     HOST i32 [n_layers+1]; dims[0] must equal L, dims[n_layers] must be 1,
  *            2 <= n_layers <= 4, hidden widths multiples of 16 and <= 256

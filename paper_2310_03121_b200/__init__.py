@@ -31,7 +31,7 @@ EXPORTS = [
     "aev_create", "aev_destroy", "aev_length", "aev_neighbors", "aev_forward", "aev_backward",
     "ani_mlp_load", "ani_mlp_set_ensemble", "ani_mlp_load_model", "ani_mlp_kernel", "ani_energy_forces", "ani_energy_forces_subset", "aev_forward_backward_host", "ani_energy_forces_host",
     "aev_export_pairs", "aev_export_counts", "aev_set_profiling", "aev_get_profile", "aev_status", "aev_launch_count", "aev_neighbor_builds", "aev_probe_fp32_tflops",
-    "aev_error_string", "aev_pairs_static",
+    "aev_error_string", "aev_pairs_static", "aev_forward_range",
 ]
 
 
@@ -89,6 +89,8 @@ def lib():
         L.aev_neighbors.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, vp]
         L.aev_forward.restype = C.c_int
         L.aev_forward.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, f32p, vp]
+        L.aev_forward_range.restype = C.c_int
+        L.aev_forward_range.argtypes = [vp, f32p, i32p, C.POINTER(C.c_float), i32, i32, i32, i32, f32p, vp]
         L.aev_backward.restype = C.c_int
         L.aev_backward.argtypes = [vp, f32p, f32p, vp]
         L.ani_mlp_load.restype = C.c_int
@@ -214,6 +216,21 @@ class Context:
                                  _dev_ptr(species, torch.int32, "species"), bp, n, batch,
                                  _dev_ptr(aev_out, torch.float32, "aev_out"), _stream(stream)),
                "aev_forward")
+        return aev_out
+
+    def aev_forward_range(self, pos, species, box, first: int, count: int, aev_out=None, stream=None):
+        """aev_forward for the central atoms [first, first + count) (flat index) only; rows outside the slab are left
+        as they are in `aev_out` (zeros if this call allocates it).  The next aev_backward returns the slab's partial
+        forces on all atoms."""
+        import torch
+        batch, n = pos.shape[0], pos.shape[1]
+        if aev_out is None:
+            aev_out = torch.zeros((batch, n, self.length), dtype=torch.float32, device=pos.device)
+        keep, bp = _box(box)
+        _check(lib().aev_forward_range(self._h, _dev_ptr(pos, torch.float32, "pos"),
+                                       _dev_ptr(species, torch.int32, "species"), bp, n, batch, int(first), int(count),
+                                       _dev_ptr(aev_out, torch.float32, "aev_out"), _stream(stream)),
+               "aev_forward_range")
         return aev_out
 
     def aev_backward(self, grad_aev, forces_out=None, stream=None):

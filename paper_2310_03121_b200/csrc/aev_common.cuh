@@ -54,6 +54,8 @@ struct Geom {
     int cap_r, cap_a;            // per-atom neighbour capacities (total radial / angular)
     int cand_cap;                // shared-memory candidate tile capacity (float4 entries)
     float box[3], inv_box[3], cell_scale[3];   // cell_scale = nc / L
+    int c_first, c_count;        // central atoms k_aev / k_backward evaluate: flat indices [c_first, c_first + c_count)
+                                 // (all of them unless aev_forward_range asked for a slab)
 };
 
 // Device workspace owned by the context.
@@ -116,6 +118,7 @@ struct aev_ctx {
     int vcap_r, vcap_a;          // per-atom capacities of the Verlet lists
     aevb::Geom vgeom;            // geometry of the last call in skin mode (a change invalidates the Verlet lists)
     int vgeom_set;
+    int next_first, next_count;  // central-atom range of the NEXT launch_neighbors (aev_forward_range); count < 0 = all
     int fwd_smem_optin;          // bytes of dynamic smem the forward kernels were opted into (per device => per ctx)
     size_t bwd_smem_optin, mlp_smem_optin;
     int tc_smem_optin;

@@ -225,3 +225,42 @@ def test_deterministic_flag_on_the_unstaged_neighbour_scan(pkg):
     assert np.abs(runs[0][0].cpu().numpy() - want_aev).max() <= AEV_TOL * np.abs(want_aev).max()
     _check_forces(runs[0][1].cpu().numpy(), want_f, what="unstaged, deterministic")
     ctx.close()
+
+
+@pytest.mark.parametrize("k_slabs", [2, 4])
+def test_slabs_of_central_atoms_add_up_to_the_full_evaluation(pkg, k_slabs):
+    """SURVEY 8(f) rank 4 (sharding over GPUs), testable on one GPU: C3 evaluated as K slabs of central atoms with
+    aev_forward_range.  Each slab's AEV rows equal the oracle's rows, rows outside the slab are not written, each
+    slab's partial forces equal the oracle's backward with the upstream gradient masked to the slab (forces are linear
+    in the gradient rows), and the partial forces add up to the full forces."""
+    from paper_2310_03121_b200.sharded import central_ranges
+    from test_gpu_parity import AEV_TOL
+    w = make_workload("C3")
+    ctx = pkg.Context(w.params, max_atoms=w.n_atoms)
+    pos, sp, g = (torch.from_numpy(x).cuda() for x in (w.pos, w.species, w.grad_aev))
+    want_a = oracle.aev_forward(w.params, w.pos, w.species, w.box, use_cells=True)
+    want_f = oracle.aev_backward(w.params, w.pos, w.species, w.box, w.grad_aev, use_cells=True)
+    scale = np.abs(want_a).max()
+    total = np.zeros_like(want_f)
+    ranges = central_ranges(w.n_atoms, k_slabs)
+    assert ranges[0][0] == 0 and sum(c for _, c in ranges) == w.n_atoms
+    for first, count in ranges:
+        out = torch.full((1, w.n_atoms, ctx.length), -3.0, dtype=torch.float32, device="cuda")
+        ctx.aev_forward_range(pos, sp, w.box, first, count, aev_out=out)
+        f = ctx.aev_backward(g)
+        ctx.check_status()
+        a = out.cpu().numpy()[0]
+        assert np.abs(a[first:first + count] - want_a[0, first:first + count]).max() <= AEV_TOL * scale
+        assert (a[:first] == -3.0).all() and (a[first + count:] == -3.0).all()
+        gm = np.zeros_like(w.grad_aev)
+        gm[0, first:first + count] = w.grad_aev[0, first:first + count]
+        want_p = oracle.aev_backward(w.params, w.pos, w.species, w.box, gm, use_cells=True)
+        _check_forces(f.cpu().numpy(), want_p, what=("slab", k_slabs, first))
+        total += f.cpu().numpy().astype(np.float64)
+    _check_forces(total, want_f, what=("slabs summed", k_slabs))
+    # the next plain call is a full evaluation again (the range does not stick)
+    ctx.aev_forward(pos, sp, w.box)
+    _check_forces(ctx.aev_backward(g).cpu().numpy(), want_f, what="full after slabs")
+    with pytest.raises(pkg.AevError):
+        ctx.aev_forward_range(pos, sp, w.box, w.n_atoms - 10, 11)
+    ctx.close()
